@@ -1,0 +1,28 @@
+"""Build the CPU oracle shared library (test infrastructure; see su_oracle.h).
+
+    python oracle/build.py            # -> oracle/liboracle.so
+
+-ffp-contract=off: the oracle evaluates the formulas as written (no FMA contraction), R19.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "su_oracle.cpp")
+LIB = os.path.join(HERE, "liboracle.so")
+FLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-Wall"]
+
+
+def build(force: bool = False) -> str:
+    deps = [SRC, os.path.join(HERE, "su_oracle.h")]
+    if (not force and os.path.exists(LIB)
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps)):
+        return LIB
+    cmd = ["g++", *FLAGS, "-o", LIB, SRC]
+    subprocess.run(cmd, check=True, cwd=HERE)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))
