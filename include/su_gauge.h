@@ -1,0 +1,139 @@
+/*
+ * su_gauge.h — C ABI of libsugauge: B200 (sm_100a) Monte Carlo generation of 4-D SU(Nc) pure-gauge
+ * (Wilson action) configurations: Cabibbo-Marinari pseudo-heatbath with Kennedy-Pendleton SU(2)
+ * draws + microcanonical overrelaxation on even/odd checkerboards, plaquette and Polyakov-loop
+ * reductions. Method: Cardoso & Bicudo, arXiv:1112.4533 ("PAPER.md" below = its text, cited by line).
+ *
+ * Conventions
+ *  - Every call returns su_status; nothing throws, aborts or exits across this boundary.
+ *    Out-parameters are written only on SU_OK. su_last_error() gives a text for the last failure.
+ *  - Pointers are HOST pointers unless the name/documentation says "device".
+ *  - A lattice handle is bound to one CUDA device and one stream; calls on one handle must not be
+ *    made concurrently from several host threads. Kernels are enqueued on the handle's stream.
+ *  - Geometry: periodic Lx x Ly x Lz x Lt lattice, every extent even and >= 2
+ *    (checkerboard + periodic boundary), site index i = x + Lx (y + Ly (z + Lz t)), directions
+ *    mu = 0..3 <-> x,y,z,t, parity = (x+y+z+t) mod 2.
+ *  - Device storage: structure of arrays
+ *        links[mu][parity][elem][cb],  cb = i / 2  (checkerboard index, x fastest),
+ *    one array of (re,im) pairs per matrix element: Nc=2 -> 2 pairs (a0,a1),(a2,a3) of eq 6
+ *    (PAPER.md:70,153); Nc=3 -> 9 pairs, or 6 pairs (first two rows) in RECON12;
+ *    Nc>=4 -> Nc^2 pairs.
+ *  - Randomness: counter-based Philox4x32-10 keyed by (seed; site, sweep, kind, pass, parity, mu,
+ *    subgroup, attempt). No RNG state is stored; (seed, sweep counter, links) determine the chain.
+ */
+#ifndef SU_GAUGE_H
+#define SU_GAUGE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default) /* the library itself is built with -fvisibility=hidden */
+#endif
+
+typedef struct su_lattice su_lattice; /* opaque, owned by the library */
+
+typedef enum {
+    SU_OK = 0,
+    SU_EINVAL = 1,       /* NULL pointer, odd or <2 extent, Nc<2, bad beta/pass counts/sizes, RECON12 with Nc!=3 */
+    SU_EUNSUPPORTED = 2, /* Nc above the generic kernel's limit (SU_MAX_NC) */
+    SU_ENOMEM = 3,       /* host or device allocation failed / caller buffer too small */
+    SU_ECUDA = 4,        /* CUDA error (sticky; text via su_last_error) */
+    SU_ESTATE = 5        /* sweep / measurement / export before init or import */
+} su_status;
+
+typedef enum { SU_FP32 = 0, SU_FP64 = 1 } su_precision;
+typedef enum { SU_STORE_FULL = 0, SU_STORE_RECON12 = 1 } su_storage; /* RECON12: Nc == 3 only */
+typedef enum {
+    SU_KERNEL_AUTO = 0,        /* specialised for Nc = 2,3,4, generic otherwise */
+    SU_KERNEL_SPECIALISED = 1, /* register-resident kernels; SU_EUNSUPPORTED for Nc > 4 */
+    SU_KERNEL_GENERIC = 2      /* the generic SU(Nc) kernel at any supported Nc */
+} su_kernel;
+
+#define SU_MAX_NC 8
+
+typedef struct {
+    su_storage storage;
+    su_kernel kernel;
+    int device;          /* CUDA device ordinal; -1 = current device */
+    void* stream;        /* cudaStream_t to enqueue on; NULL = the legacy default stream */
+    void* buffer;        /* DEVICE pointer to caller-owned link storage (e.g. a torch uint8 tensor),
+                            256-byte aligned, or NULL: the library allocates. Must outlive the handle. */
+    size_t buffer_bytes; /* size of buffer; must be >= su_lattice_bytes(...) */
+} su_options;
+
+/* Bytes of device link storage for this lattice: 4 V * R * sizeof(real), R = reals per link
+ * (4 / 18 / 12 / 2 Nc^2), rounded up to 256. Returns 0 on invalid arguments. */
+size_t su_lattice_bytes(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, su_storage s);
+
+/* Create a lattice. The links are undefined until su_init_* / su_import_links. */
+su_status su_lattice_create(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, su_lattice** out);
+su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p,
+                               const su_options* opt, su_lattice** out);
+su_status su_lattice_destroy(su_lattice*); /* synchronises the stream; frees what the library owns */
+
+/* Cold start: all links = identity. Sets the RNG seed, sweep counter = 0. */
+su_status su_init_cold(su_lattice*, uint64_t seed);
+/* Hot start: independent Haar-random SU(Nc) links drawn from Philox(seed);
+ * sweep counter = 0. Asynchronous on the stream. */
+su_status su_init_hot(su_lattice*, uint64_t seed);
+
+/* One Monte Carlo sweep: n_heatbath (pseudo-)heatbath passes
+ * (eqs 9-16) followed by n_overrelax overrelaxation passes (eq 17); each pass updates every link
+ * once, as 8 sub-steps: parity 0,1 (outer) x mu 0..3 (inner). Wilson coupling beta = 2Nc/g^2
+ * (eq 3). Asynchronous on the stream. Uses, then increments, the handle's sweep counter.
+ * Never reunitarises. 0 <= n_heatbath <= 255, n_overrelax >= 0, beta finite and >= 0. */
+su_status su_sweep(su_lattice*, double beta, int n_heatbath, int n_overrelax);
+
+/* Mean plaquette <ReTr P>/Nc over the 6V plaquettes (eq 4); fp64 accumulation.
+ * Synchronises the stream. Cold start gives exactly 1. */
+su_status su_plaquette(su_lattice*, double* out);
+/* Polyakov loop: mean over spatial sites of Tr prod_{t} U_3(x,t) / Nc; out = {re, im}. Synchronises. */
+su_status su_polyakov(su_lattice*, double out[2]);
+/* Project every link back to SU(Nc): Nc=2 normalise; Nc=3 Gram-Schmidt on
+ * rows 0,1 + cross product; Nc>=4 Gram-Schmidt + phase on the last row. Asynchronous. */
+su_status su_reunitarize(su_lattice*);
+
+/* Copy the links to / from a HOST array of doubles in the canonical layout
+ * [t][z][y][x][mu][row][col][re,im]; n_doubles must equal 4 V * 2 Nc^2. RECON12 rebuilds / drops
+ * the third row. Synchronise. su_import_links marks the lattice initialised. */
+su_status su_export_links(su_lattice*, double* host_dst, size_t n_doubles);
+su_status su_import_links(su_lattice*, const double* host_src, size_t n_doubles);
+
+/* ---- test / resume hooks ---- */
+/* Set the RNG seed and sweep counter: export + su_set_rng + import is an exact resume. */
+su_status su_set_rng(su_lattice*, uint64_t seed, uint32_t sweep_counter);
+/* One sub-step of a sweep: kind 0 = heatbath, 1 = overrelaxation; pass = heatbath pass number
+ * (RNG counter field); parity 0/1; mu 0..3. host_attempts: NULL, or n_sub * V/2 bytes receiving
+ * the Kennedy-Pendleton attempts used per [subgroup][cb] (0 = none / exhausted); when given the
+ * call synchronises. Does not touch the sweep counter. */
+su_status su_substep(su_lattice*, double beta, int kind, int pass, int parity, int mu, uint8_t* host_attempts);
+/* Totals since the last init: KP attempts used, and subgroup draws abandoned after 1024 attempts
+ * or a null projection (those leave the link unchanged for that subgroup). Synchronises. */
+su_status su_get_counters(su_lattice*, uint64_t* kp_attempts_total, uint64_t* kp_exhausted);
+/* Stream synchronise (surfaces asynchronous errors). */
+su_status su_synchronize(su_lattice*);
+/* Per-handle toggle: capture each distinct (beta, n_hb, n_or) sweep into a CUDA graph and replay it
+ * (launch-bound small lattices). Default off. */
+su_status su_set_graph_mode(su_lattice*, int enabled);
+/* Per-kind device timing of su_sweep (for the benchmark's roofline): when enabled (and graph mode
+ * is off) su_sweep records CUDA events on the handle's stream before the heatbath passes, between
+ * the heatbath and overrelaxation passes, and after; su_get_timing synchronises and returns the
+ * accumulated milliseconds and update-kernel launches per kind since su_set_timing. */
+su_status su_set_timing(su_lattice*, int enabled);
+su_status su_get_timing(su_lattice*, double* hb_ms, uint64_t* hb_launches, double* or_ms, uint64_t* or_launches);
+/* Number of kernels this handle has launched so far (for the benchmark's gpu_launches). */
+su_status su_get_launch_count(su_lattice*, uint64_t* out);
+
+/* Text of the last error on this handle ("" if none); static text if the handle is NULL.
+ * Owned by the library, valid until the next call on the handle. */
+const char* su_last_error(const su_lattice*);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif

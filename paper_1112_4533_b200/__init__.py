@@ -1,0 +1,229 @@
+"""paper_1112_4533_b200 — thin Python binding of libsugauge (include/su_gauge.h).
+
+Argument marshalling only: every step of the path (staple, Cabibbo-Marinari heatbath with
+Kennedy-Pendleton draws, overrelaxation, plaquette / Polyakov reductions, reunitarisation, init,
+import / export layout conversion) runs in the CUDA kernels under csrc/. PyTorch supplies device
+memory (a uint8 tensor that backs the links) and the stream; nothing here computes, and there is
+no CPU fallback: a missing library or a missing GPU raises.
+
+Method: Cardoso & Bicudo, arXiv:1112.4533.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsugauge.so")
+
+SU_OK, SU_EINVAL, SU_EUNSUPPORTED, SU_ENOMEM, SU_ECUDA, SU_ESTATE = range(6)
+_STATUS = {0: "SU_OK", 1: "SU_EINVAL", 2: "SU_EUNSUPPORTED", 3: "SU_ENOMEM", 4: "SU_ECUDA", 5: "SU_ESTATE"}
+SU_FP32, SU_FP64 = 0, 1
+SU_STORE_FULL, SU_STORE_RECON12 = 0, 1
+SU_KERNEL_AUTO, SU_KERNEL_SPECIALISED, SU_KERNEL_GENERIC = 0, 1, 2
+SU_MAX_NC = 8
+
+# every entry point include/su_gauge.h declares (tests check the library exports exactly these)
+ABI_SYMBOLS = (
+    "su_lattice_bytes", "su_lattice_create", "su_lattice_create_ex", "su_lattice_destroy",
+    "su_init_cold", "su_init_hot", "su_sweep", "su_plaquette", "su_polyakov", "su_reunitarize",
+    "su_export_links", "su_import_links", "su_set_rng", "su_substep", "su_get_counters",
+    "su_synchronize", "su_set_graph_mode", "su_set_timing", "su_get_timing", "su_get_launch_count", "su_last_error",
+)
+
+
+class su_options(C.Structure):
+    _fields_ = [("storage", C.c_int), ("kernel", C.c_int), ("device", C.c_int), ("stream", C.c_void_p),
+                ("buffer", C.c_void_p), ("buffer_bytes", C.c_size_t)]
+
+
+class SuError(RuntimeError):
+    def __init__(self, status, what, detail=""):
+        self.status = status
+        super().__init__(f"{what}: {_STATUS.get(status, status)}" + (f" ({detail})" if detail else ""))
+
+
+_lib = None
+
+
+def lib():
+    """Load libsugauge.so (built in-tree by `python -m paper_1112_4533_b200.build`). Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1112_4533_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    P, I, D = C.c_void_p, C.c_int, C.c_double
+    L.su_lattice_bytes.argtypes = [I] * 7
+    L.su_lattice_bytes.restype = C.c_size_t
+    L.su_lattice_create.argtypes = [I] * 6 + [C.POINTER(P)]
+    L.su_lattice_create_ex.argtypes = [I] * 6 + [C.POINTER(su_options), C.POINTER(P)]
+    L.su_lattice_destroy.argtypes = [P]
+    L.su_init_cold.argtypes = [P, C.c_uint64]
+    L.su_init_hot.argtypes = [P, C.c_uint64]
+    L.su_sweep.argtypes = [P, D, I, I]
+    L.su_plaquette.argtypes = [P, C.POINTER(D)]
+    L.su_polyakov.argtypes = [P, C.POINTER(D)]
+    L.su_reunitarize.argtypes = [P]
+    L.su_export_links.argtypes = [P, C.c_void_p, C.c_size_t]
+    L.su_import_links.argtypes = [P, C.c_void_p, C.c_size_t]
+    L.su_set_rng.argtypes = [P, C.c_uint64, C.c_uint32]
+    L.su_substep.argtypes = [P, D, I, I, I, I, C.c_void_p]
+    L.su_get_counters.argtypes = [P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.su_synchronize.argtypes = [P]
+    L.su_set_graph_mode.argtypes = [P, I]
+    L.su_set_timing.argtypes = [P, I]
+    L.su_get_timing.argtypes = [P, C.POINTER(D), C.POINTER(C.c_uint64), C.POINTER(D), C.POINTER(C.c_uint64)]
+    L.su_get_launch_count.argtypes = [P, C.POINTER(C.c_uint64)]
+    L.su_last_error.argtypes = [P]
+    L.su_last_error.restype = C.c_char_p
+    for name in ABI_SYMBOLS:
+        if name not in ("su_lattice_bytes", "su_last_error"):
+            getattr(L, name).restype = I
+    _lib = L
+    return L
+
+
+def _prec(precision):
+    if precision in ("fp64", "f64", "double"):
+        return SU_FP64
+    if precision in ("fp32", "f32", "float"):
+        return SU_FP32
+    raise ValueError(f"precision must be 'fp32' or 'fp64', got {precision!r}")
+
+
+def lattice_bytes(Nc, dims, precision="fp64", recon12=False):
+    return lib().su_lattice_bytes(Nc, *dims, _prec(precision), SU_STORE_RECON12 if recon12 else SU_STORE_FULL)
+
+
+class Lattice:
+    """One SU(Nc) gauge field on the GPU. Same method names as the C ABI without the su_ prefix.
+
+    dims = (Lx, Ly, Lz, Lt). kernel: 'auto' | 'specialised' | 'generic'. The link storage is a torch
+    uint8 tensor on `device`, kernels run on torch's current stream at construction time.
+    """
+
+    def __init__(self, Nc, dims, precision="fp64", recon12=False, kernel="auto", device=0, graph=False):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1112_4533_b200 needs a CUDA device (there is no CPU fallback)")
+        L = lib()
+        self.Nc, self.dims = int(Nc), tuple(int(d) for d in dims)
+        self.precision = "fp64" if _prec(precision) == SU_FP64 else "fp32"
+        self.recon12 = bool(recon12)
+        self.V = int(np.prod(self.dims))
+        self.n_sub = self.Nc * (self.Nc - 1) // 2
+        self._h = C.c_void_p()
+        self._torch = torch
+        self.device = torch.device("cuda", device) if isinstance(device, int) else torch.device(device)
+        storage = SU_STORE_RECON12 if recon12 else SU_STORE_FULL
+        nbytes = L.su_lattice_bytes(self.Nc, *self.dims, _prec(precision), storage)
+        if nbytes == 0:
+            raise SuError(SU_EINVAL, "su_lattice_bytes", "invalid Nc / extents / storage")
+        with torch.cuda.device(self.device):
+            self.buffer = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = torch.cuda.current_stream(self.device)
+        opt = su_options(storage, {"auto": 0, "specialised": 1, "generic": 2}[kernel], self.device.index or 0,
+                         C.c_void_p(self.stream.cuda_stream), C.c_void_p(self.buffer.data_ptr()), nbytes)
+        st = L.su_lattice_create_ex(self.Nc, *self.dims, _prec(precision), C.byref(opt), C.byref(self._h))
+        if st != SU_OK:
+            self._h = C.c_void_p()
+            raise SuError(st, "su_lattice_create_ex")
+        if graph:
+            self.set_graph_mode(True)
+
+    # ---- plumbing ----
+    def _ck(self, st, what):
+        if st != SU_OK:
+            msg = lib().su_last_error(self._h)
+            raise SuError(st, what, msg.decode() if msg else "")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().su_lattice_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # ---- the C ABI, one to one ----
+    def init_cold(self, seed):
+        self._ck(lib().su_init_cold(self._h, seed), "su_init_cold")
+
+    def init_hot(self, seed):
+        self._ck(lib().su_init_hot(self._h, seed), "su_init_hot")
+
+    def set_rng(self, seed, sweep_counter):
+        self._ck(lib().su_set_rng(self._h, seed, sweep_counter), "su_set_rng")
+
+    def sweep(self, beta, n_hb=1, n_or=4):
+        self._ck(lib().su_sweep(self._h, beta, n_hb, n_or), "su_sweep")
+
+    def substep(self, beta, kind, pass_, parity, mu, want_attempts=False):
+        att = np.zeros((self.n_sub, self.V // 2), dtype=np.uint8) if want_attempts else None
+        self._ck(lib().su_substep(self._h, beta, kind, pass_, parity, mu, att.ctypes.data if want_attempts else None),
+                 "su_substep")
+        return att
+
+    def plaquette(self):
+        out = C.c_double()
+        self._ck(lib().su_plaquette(self._h, C.byref(out)), "su_plaquette")
+        return out.value
+
+    def polyakov(self):
+        out = (C.c_double * 2)()
+        self._ck(lib().su_polyakov(self._h, out), "su_polyakov")
+        return complex(out[0], out[1])
+
+    def reunitarize(self):
+        self._ck(lib().su_reunitarize(self._h), "su_reunitarize")
+
+    def export_links(self, out=None):
+        """-> complex128 array [t][z][y][x][mu][row][col] (host)"""
+        Lx, Ly, Lz, Lt = self.dims
+        if out is None:
+            out = np.empty((Lt, Lz, Ly, Lx, 4, self.Nc, self.Nc), dtype=np.complex128)
+        self._ck(lib().su_export_links(self._h, out.ctypes.data, out.size * 2), "su_export_links")
+        return out
+
+    def import_links(self, links):
+        a = np.ascontiguousarray(links, dtype=np.complex128)
+        self._ck(lib().su_import_links(self._h, a.ctypes.data, a.size * 2), "su_import_links")
+
+    def counters(self):
+        a, e = C.c_uint64(), C.c_uint64()
+        self._ck(lib().su_get_counters(self._h, C.byref(a), C.byref(e)), "su_get_counters")
+        return a.value, e.value
+
+    def synchronize(self):
+        self._ck(lib().su_synchronize(self._h), "su_synchronize")
+
+    def set_graph_mode(self, enabled):
+        self._ck(lib().su_set_graph_mode(self._h, int(bool(enabled))), "su_set_graph_mode")
+
+    def set_timing(self, enabled):
+        self._ck(lib().su_set_timing(self._h, int(bool(enabled))), "su_set_timing")
+
+    def timing(self):
+        """-> dict(hb_ms, hb_launches, or_ms, or_launches) accumulated since set_timing(True)"""
+        a, b = C.c_double(), C.c_double()
+        na, nb = C.c_uint64(), C.c_uint64()
+        self._ck(lib().su_get_timing(self._h, C.byref(a), C.byref(na), C.byref(b), C.byref(nb)), "su_get_timing")
+        return {"hb_ms": a.value, "hb_launches": na.value, "or_ms": b.value, "or_launches": nb.value}
+
+    def launch_count(self):
+        n = C.c_uint64()
+        self._ck(lib().su_get_launch_count(self._h, C.byref(n)), "su_get_launch_count")
+        return n.value

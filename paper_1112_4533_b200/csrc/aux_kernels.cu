@@ -1,0 +1,364 @@
+// aux_kernels.cu — everything on the path except the link update: plaquette and Polyakov-loop
+// reductions (fp64 accumulation, warp shuffle + block + final pass), reunitarisation, cold / hot
+// start, and the SoA <-> canonical-layout conversion used by export / import.
+// Compiled once per colour count with -DSUG_NC=<Nc>.
+#include "su_internal.h"
+
+#ifndef SUG_NC
+#error "compile with -DSUG_NC=<Nc>"
+#endif
+
+namespace sug {
+
+#define SUG_CAT_(a, b) a##b
+#define SUG_CAT(a, b) SUG_CAT_(a, b)
+
+// ------------------------------------------------------------------------------------------
+// Plaquette (eq 4): per site the six P_mu,nu; Re Tr P = Re Tr[(U_mu(x) U_nu(x+mu))
+// (U_nu(x) U_mu(x+nu))^dagger]. Products in T, site sum and reduction in double.
+// ------------------------------------------------------------------------------------------
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(REDUCE_BLOCK) k_plaquette(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    typedef Mat<NC, T, UNR> M;
+    typedef cx<T> C;
+    const unsigned idx = blockIdx.x * REDUCE_BLOCK + threadIdx.x;
+    double acc = 0.0;
+    if (idx < 2u * a.g.Vh) {
+        const unsigned Vh = a.g.Vh;
+        const int p = idx >= Vh ? 1 : 0;
+        const unsigned cb = idx - (p ? Vh : 0u);
+        int c[4];
+        decode_cb(a.g, cb, p, c);
+        unsigned fwd[4];
+#pragma unroll
+        for (int d = 0; d < 4; ++d) fwd[d] = cb_shift(a.g, c, d, +1);
+        C A[NC * NC], B[NC * NC], P[NC * NC], Q[NC * NC];
+#pragma unroll 1
+        for (int mu = 0; mu < 3; ++mu)
+#pragma unroll 1
+            for (int nu = mu + 1; nu < 4; ++nu) {
+                IO::template load<true>(IO::plane((const void*)a.links, a.g, mu, p), Vh, cb, A);
+                IO::template load<true>(IO::plane((const void*)a.links, a.g, nu, 1 - p), Vh, fwd[mu], B);
+                M::mul_nn(A, B, P);
+                IO::template load<true>(IO::plane((const void*)a.links, a.g, nu, p), Vh, cb, A);
+                IO::template load<true>(IO::plane((const void*)a.links, a.g, mu, 1 - p), Vh, fwd[nu], B);
+                M::mul_nn(A, B, Q);
+                acc += (double)M::retr_nd(P, Q);
+            }
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) a.partials[blockIdx.x] = acc;
+}
+
+// Polyakov loop (reading R9): per spatial site Tr prod_t U_3(x,t); complex, double accumulation.
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(REDUCE_BLOCK) k_polyakov(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    typedef Mat<NC, T, UNR> M;
+    typedef cx<T> C;
+    const unsigned Vs = (unsigned)a.g.L[0] * a.g.L[1] * a.g.L[2];
+    const unsigned xs = blockIdx.x * REDUCE_BLOCK + threadIdx.x;
+    double re = 0.0, im = 0.0;
+    if (xs < Vs) {
+        const int x = (int)(xs % (unsigned)a.g.L[0]);
+        const int y = (int)((xs / (unsigned)a.g.L[0]) % (unsigned)a.g.L[1]);
+        const int z = (int)(xs / ((unsigned)a.g.L[0] * a.g.L[1]));
+        C P[NC * NC], A[NC * NC], Q[NC * NC];
+        IO::template load<true>(IO::plane((const void*)a.links, a.g, 3, (x + y + z) & 1), a.g.Vh, cb_of(a.g, x, y, z, 0), P);
+#pragma unroll 1
+        for (int t = 1; t < a.g.L[3]; ++t) {
+            IO::template load<true>(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), a.g.Vh, cb_of(a.g, x, y, z, t), A);
+            M::mul_nn(P, A, Q);
+#pragma unroll(UNR ? NC * NC : 1)
+            for (int e = 0; e < NC * NC; ++e) P[e] = Q[e];
+        }
+#pragma unroll(UNR ? NC : 1)
+        for (int d = 0; d < NC; ++d) { re += (double)P[d * NC + d].re; im += (double)P[d * NC + d].im; }
+    }
+    re = block_sum(re);
+    im = block_sum(im);
+    if (threadIdx.x == 0) { a.partials[blockIdx.x] = re; a.partials[gridDim.x + blockIdx.x] = im; }
+}
+
+// Final pass: result[c] = scale * sum_b partials[c * nb + b], c < ncomp. One block; fixed order.
+static __global__ void __launch_bounds__(REDUCE_BLOCK) k_reduce_final(const double* __restrict__ partials, unsigned nb,
+                                                               int ncomp, double scale, double* __restrict__ result) {
+    for (int c = 0; c < ncomp; ++c) {
+        double s = 0.0;
+        for (unsigned i = threadIdx.x; i < nb; i += REDUCE_BLOCK) s += partials[(size_t)c * nb + i];
+        s = block_sum(s);
+        if (threadIdx.x == 0) result[c] = s * scale;
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Gram-Schmidt / determinant on a local matrix (rolled loops), used by reunitarise (Nc >= 4)
+// and by the hot start (always double, reading R20).
+// ------------------------------------------------------------------------------------------
+template <int NC, class R>
+__device__ void gram_schmidt_rows(cx<R>* U, int nrows) {
+#pragma unroll 1
+    for (int r = 0; r < nrows; ++r) {
+#pragma unroll 1
+        for (int p = 0; p < r; ++p) {
+            cx<R> dot = mk<R>(0, 0);
+            for (int k = 0; k < NC; ++k) mad_ca(dot, U[p * NC + k], U[r * NC + k]);
+            for (int k = 0; k < NC; ++k) U[r * NC + k] = U[r * NC + k] - dot * U[p * NC + k];
+        }
+        R n2 = 0;
+        for (int k = 0; k < NC; ++k) n2 += U[r * NC + k].re * U[r * NC + k].re + U[r * NC + k].im * U[r * NC + k].im;
+        R inv = (R)1 / Fn<R>::sqrt(n2);
+        for (int k = 0; k < NC; ++k) U[r * NC + k] = inv * U[r * NC + k];
+    }
+}
+
+template <int NC, class R>
+__device__ cx<R> determinant(const cx<R>* A) {
+    cx<R> Mx[NC * NC];
+    for (int e = 0; e < NC * NC; ++e) Mx[e] = A[e];
+    cx<R> det = mk<R>(1, 0);
+#pragma unroll 1
+    for (int c = 0; c < NC; ++c) {
+        int p = c;
+        R best = Mx[c * NC + c].re * Mx[c * NC + c].re + Mx[c * NC + c].im * Mx[c * NC + c].im;
+        for (int r = c + 1; r < NC; ++r) {
+            R m = Mx[r * NC + c].re * Mx[r * NC + c].re + Mx[r * NC + c].im * Mx[r * NC + c].im;
+            if (m > best) { best = m; p = r; }
+        }
+        if (best == (R)0) return mk<R>(0, 0);
+        if (p != c) {
+            for (int k = 0; k < NC; ++k) { cx<R> t = Mx[p * NC + k]; Mx[p * NC + k] = Mx[c * NC + k]; Mx[c * NC + k] = t; }
+            det = mk<R>(-det.re, -det.im);
+        }
+        det = det * Mx[c * NC + c];
+        const cx<R> pinv = (1 / best) * conj(Mx[c * NC + c]);
+        for (int r = c + 1; r < NC; ++r) {
+            cx<R> f = Mx[r * NC + c] * pinv;
+            for (int k = c; k < NC; ++k) Mx[r * NC + k] = Mx[r * NC + k] - f * Mx[c * NC + k];
+        }
+    }
+    return det;
+}
+
+template <int NC, class R>
+__device__ void fix_determinant_phase(cx<R>* U) {          // last row *= conj(det)/|det|
+    cx<R> d = determinant<NC, R>(U);
+    R inv = (R)1 / Fn<R>::sqrt(d.re * d.re + d.im * d.im);
+    cx<R> ph = mk<R>(d.re * inv, -d.im * inv);
+    for (int k = 0; k < NC; ++k) U[(NC - 1) * NC + k] = U[(NC - 1) * NC + k] * ph;
+}
+
+// one thread per link; idx = plane * Vh + cb so that stores coalesce
+__device__ __forceinline__ bool link_of_thread(const Geom& g, unsigned idx, int& mu, int& p, unsigned& cb) {
+    if (idx >= 8u * g.Vh) return false;
+    unsigned plane = idx / g.Vh;
+    cb = idx - plane * g.Vh;
+    mu = (int)(plane >> 1);
+    p = (int)(plane & 1u);
+    return true;
+}
+
+// Reunitarisation (reading R10), arithmetic in T.
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    int mu, p; unsigned cb;
+    if (!link_of_thread(a.g, blockIdx.x * 128u + threadIdx.x, mu, p, cb)) return;
+    typename IO::T2* pl = IO::plane(a.links, a.g, mu, p);
+    cx<T> U[NC * NC];
+    IO::template load<false>(pl, a.g.Vh, cb, U);
+    if (NC == 2) {
+        T n = Fn<T>::sqrt((U[0].re * U[0].re + U[0].im * U[0].im) + (U[1].re * U[1].re + U[1].im * U[1].im));
+        U[0] = mk<T>(U[0].re / n, U[0].im / n);
+        U[1] = mk<T>(U[1].re / n, U[1].im / n);
+    } else if (NC == 3) {
+        gram_schmidt_rows<NC, T>(U, 2);
+        su3_third_row(U);
+    } else {
+        gram_schmidt_rows<NC, T>(U, NC);
+        fix_determinant_phase<NC, T>(U);
+    }
+    IO::store(pl, a.g.Vh, cb, U);
+}
+
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(128) k_init_cold(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    int mu, p; unsigned cb;
+    if (!link_of_thread(a.g, blockIdx.x * 128u + threadIdx.x, mu, p, cb)) return;
+    cx<T> U[NC * NC];
+    for (int i = 0; i < NC; ++i)
+        for (int j = 0; j < NC; ++j) U[i * NC + j] = mk<T>(i == j ? (T)1 : (T)0, (T)0);
+    IO::store(IO::plane(a.links, a.g, mu, p), a.g.Vh, cb, U);
+}
+
+// Hot start (readings R12, R20): Haar SU(Nc) per link from Philox blocks
+// (kind 2, c0 = site, c1 = 0, c3 = block): uniforms in fours -> Box-Muller pairs -> 2Nc^2 Gaussians
+// row-major (re,im) -> modified Gram-Schmidt -> last row * conj(det)/|det|. Nc = 2: the first four
+// Gaussians, normalised, are (a0..a3). Computed in double, rounded to T on store.
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(128) k_init_hot(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    int mu, p; unsigned cb;
+    if (!link_of_thread(a.g, blockIdx.x * 128u + threadIdx.x, mu, p, cb)) return;
+    int c[4];
+    decode_cb(a.g, cb, p, c);
+    const uint32_t site = lex_of(a.g, c);
+    constexpr int NG = (NC == 2) ? 4 : 2 * NC * NC;
+    constexpr int NB = (NG + 3) / 4;
+    const double TWO_PI = 6.283185307179586476925286766559;
+    double g[NB * 4];
+#pragma unroll 1
+    for (int b = 0; b < NB; ++b) {
+        uint32_t w[4];
+        philox4x32_10(site, 0u, pack_c2(RNG_HOT, 0, p, mu, 0), (uint32_t)b, a.k0, a.k1, w);
+        for (int h = 0; h < 2; ++h) {
+            double ua = uniform01<double>(w[2 * h]), ub = uniform01<double>(w[2 * h + 1]);
+            double rad = ::sqrt(-2.0 * ::log(ua));
+            double s, co;
+            ::sincos(TWO_PI * ub, &s, &co);
+            g[4 * b + 2 * h] = rad * co;
+            g[4 * b + 2 * h + 1] = rad * s;
+        }
+    }
+    cx<double> Md[NC * NC];
+    if (NC == 2) {
+        double n = ::sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2] + g[3] * g[3]);
+        double a0 = g[0] / n, a1 = g[1] / n, a2 = g[2] / n, a3 = g[3] / n;
+        Md[0] = mk<double>(a0, a3); Md[1] = mk<double>(a2, a1);
+        Md[NC * NC - 2] = mk<double>(-a2, a1); Md[NC * NC - 1] = mk<double>(a0, -a3);
+    } else {
+        for (int e = 0; e < NC * NC; ++e) Md[e] = mk<double>(g[2 * e], g[2 * e + 1]);
+        gram_schmidt_rows<NC, double>(Md, NC);
+        fix_determinant_phase<NC, double>(Md);
+    }
+    cx<T> U[NC * NC];
+    for (int e = 0; e < NC * NC; ++e) U[e] = mk<T>((T)Md[e].re, (T)Md[e].im);
+    IO::store(IO::plane(a.links, a.g, mu, p), a.g.Vh, cb, U);
+}
+
+// SoA -> canonical [site][mu][row][col][re,im] doubles for lexicographic sites [site0, site0+nsites)
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(128) k_export(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    const unsigned l = blockIdx.x * 128u + threadIdx.x;      // local link index = (site - site0) * 4 + mu
+    if (l >= a.nsites * 4u) return;
+    const unsigned s = a.site0 + (l >> 2);
+    const int mu = (int)(l & 3u);
+    const int x = (int)(s % (unsigned)a.g.L[0]);
+    unsigned r = s / (unsigned)a.g.L[0];
+    const int y = (int)(r % (unsigned)a.g.L[1]); r /= (unsigned)a.g.L[1];
+    const int z = (int)(r % (unsigned)a.g.L[2]);
+    const int t = (int)(r / (unsigned)a.g.L[2]);
+    const int p = (x + y + z + t) & 1;
+    cx<T> U[NC * NC];
+    IO::template load<false>(IO::plane((const void*)a.links, a.g, mu, p), a.g.Vh, s >> 1, U);
+    double2* dst = (double2*)a.staging + (size_t)l * NC * NC;
+    for (int e = 0; e < NC * NC; ++e) dst[e] = make_double2((double)U[e].re, (double)U[e].im);
+}
+
+template <int NC, class T, int STORE, bool UNR>
+__global__ void __launch_bounds__(128) k_import(const AuxArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    const unsigned l = blockIdx.x * 128u + threadIdx.x;
+    if (l >= a.nsites * 4u) return;
+    const unsigned s = a.site0 + (l >> 2);
+    const int mu = (int)(l & 3u);
+    const int x = (int)(s % (unsigned)a.g.L[0]);
+    unsigned r = s / (unsigned)a.g.L[0];
+    const int y = (int)(r % (unsigned)a.g.L[1]); r /= (unsigned)a.g.L[1];
+    const int z = (int)(r % (unsigned)a.g.L[2]);
+    const int t = (int)(r / (unsigned)a.g.L[2]);
+    const int p = (x + y + z + t) & 1;
+    const double2* src = (const double2*)a.staging + (size_t)l * NC * NC;
+    cx<T> U[NC * NC];
+    for (int e = 0; e < NC * NC; ++e) { double2 v = src[e]; U[e] = mk<T>((T)v.x, (T)v.y); }
+    IO::store(IO::plane(a.links, a.g, mu, p), a.g.Vh, s >> 1, U);
+}
+
+// ---- dispatch -----------------------------------------------------------------------------
+// Reunitarise / init / import / export use rolled loops over local arrays for every Nc
+// (Gram-Schmidt and the pivoted determinant need dynamic row indices; none of them is hot).
+#define SUG_AUX_DISPATCH(KERNEL, GRID, BLOCK)                                                              \
+    do {                                                                                                   \
+        constexpr int NC = SUG_NC;                                                                         \
+        constexpr int ST0 = (NC == 2 ? STORE_QUAT : STORE_FULL);                                           \
+        constexpr int ST1 = (NC == 3 ? STORE_RECON12 : ST0);                                               \
+        const bool f64 = v.prec == SU_FP64;                                                                \
+        if (NC == 3 && v.store == STORE_RECON12) {                                                         \
+            if (f64) KERNEL<NC, double, ST1, false><<<GRID, BLOCK, 0, st>>>(a);                            \
+            else     KERNEL<NC, float,  ST1, false><<<GRID, BLOCK, 0, st>>>(a);                            \
+        } else {                                                                                           \
+            if (f64) KERNEL<NC, double, ST0, false><<<GRID, BLOCK, 0, st>>>(a);                            \
+            else     KERNEL<NC, float,  ST0, false><<<GRID, BLOCK, 0, st>>>(a);                            \
+        }                                                                                                  \
+        ++*n_launch;                                                                                       \
+    } while (0)
+
+// measurement kernels: unrolled for the specialised variants of Nc <= 4
+#define SUG_MEAS_DISPATCH(KERNEL, GRID, BLOCK)                                                                  \
+    do {                                                                                                        \
+        constexpr int NC = SUG_NC;                                                                              \
+        constexpr bool CAN_UNR = NC <= 4;                                                                       \
+        constexpr int ST0 = (NC == 2 ? STORE_QUAT : STORE_FULL);                                                \
+        constexpr int ST1 = (NC == 3 ? STORE_RECON12 : ST0);                                                    \
+        const bool f64 = v.prec == SU_FP64;                                                                     \
+        const bool unr = CAN_UNR && !v.generic;                                                                 \
+        const bool r12 = (NC == 3 && v.store == STORE_RECON12);                                                 \
+        if (unr) {                                                                                              \
+            if (r12) { if (f64) KERNEL<NC, double, ST1, CAN_UNR><<<GRID, BLOCK, 0, st>>>(a); else KERNEL<NC, float, ST1, CAN_UNR><<<GRID, BLOCK, 0, st>>>(a); } \
+            else     { if (f64) KERNEL<NC, double, ST0, CAN_UNR><<<GRID, BLOCK, 0, st>>>(a); else KERNEL<NC, float, ST0, CAN_UNR><<<GRID, BLOCK, 0, st>>>(a); } \
+        } else {                                                                                                \
+            if (r12) { if (f64) KERNEL<NC, double, ST1, false><<<GRID, BLOCK, 0, st>>>(a); else KERNEL<NC, float, ST1, false><<<GRID, BLOCK, 0, st>>>(a); }     \
+            else     { if (f64) KERNEL<NC, double, ST0, false><<<GRID, BLOCK, 0, st>>>(a); else KERNEL<NC, float, ST0, false><<<GRID, BLOCK, 0, st>>>(a); }     \
+        }                                                                                                       \
+        ++*n_launch;                                                                                            \
+    } while (0)
+
+cudaError_t SUG_CAT(plaquette_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned nb = reduce_blocks(2u * a.g.Vh);
+    SUG_MEAS_DISPATCH(k_plaquette, nb, REDUCE_BLOCK);
+    const double scale = 1.0 / (6.0 * 2.0 * (double)a.g.Vh * (double)SUG_NC);
+    k_reduce_final<<<1, REDUCE_BLOCK, 0, st>>>(a.partials, nb, 1, scale, a.result);
+    ++*n_launch;
+    return cudaGetLastError();
+}
+
+cudaError_t SUG_CAT(polyakov_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned Vs = (unsigned)a.g.L[0] * a.g.L[1] * a.g.L[2];
+    const unsigned nb = reduce_blocks(Vs);
+    SUG_MEAS_DISPATCH(k_polyakov, nb, REDUCE_BLOCK);
+    k_reduce_final<<<1, REDUCE_BLOCK, 0, st>>>(a.partials, nb, 2, 1.0 / ((double)Vs * (double)SUG_NC), a.result);
+    ++*n_launch;
+    return cudaGetLastError();
+}
+
+cudaError_t SUG_CAT(reunit_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned grid = (8u * a.g.Vh + 127u) / 128u;
+    SUG_AUX_DISPATCH(k_reunit, grid, 128);
+    return cudaGetLastError();
+}
+cudaError_t SUG_CAT(init_cold_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned grid = (8u * a.g.Vh + 127u) / 128u;
+    SUG_AUX_DISPATCH(k_init_cold, grid, 128);
+    return cudaGetLastError();
+}
+cudaError_t SUG_CAT(init_hot_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned grid = (8u * a.g.Vh + 127u) / 128u;
+    SUG_AUX_DISPATCH(k_init_hot, grid, 128);
+    return cudaGetLastError();
+}
+cudaError_t SUG_CAT(export_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned grid = (a.nsites * 4u + 127u) / 128u;
+    SUG_AUX_DISPATCH(k_export, grid, 128);
+    return cudaGetLastError();
+}
+cudaError_t SUG_CAT(import_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+    const unsigned grid = (a.nsites * 4u + 127u) / 128u;
+    SUG_AUX_DISPATCH(k_import, grid, 128);
+    return cudaGetLastError();
+}
+
+}  // namespace sug

@@ -1,0 +1,484 @@
+// su_api.cu — the C ABI of libsugauge (include/su_gauge.h): handle, validation, sweep schedule,
+// reductions' host side, import/export staging. All arithmetic of the method runs in the kernels
+// of update_kernels.cu / aux_kernels.cu; nothing here falls back to the CPU.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <tuple>
+#include <vector>
+
+#include "su_internal.h"
+
+using namespace sug;
+
+struct su_lattice {
+    int Nc = 0;
+    Geom g{};
+    size_t V = 0;
+    su_precision prec = SU_FP64;
+    Variant var{};
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    void* links = nullptr;
+    bool owns_links = false;
+    size_t links_bytes = 0;
+    double* d_partials = nullptr;
+    double* d_result = nullptr;
+    unsigned long long* d_counters = nullptr;
+    uint32_t* d_sweep = nullptr;
+    uint8_t* d_attempts = nullptr;
+    double* d_staging = nullptr;
+    size_t staging_bytes = 0;
+    uint64_t seed = 0;
+    uint32_t sweep = 0;
+    bool ready = false;
+    bool graph_mode = false;
+    std::map<std::tuple<double, int, int>, cudaGraphExec_t> graphs;
+    uint64_t n_launch = 0;
+    // per-kind device timing of su_sweep (su_set_timing): events before / between / after the pass groups
+    bool timing = false;
+    struct SweepEvents { cudaEvent_t e[3]; int n_hb, n_or; };
+    std::vector<SweepEvents> pending;
+    std::vector<cudaEvent_t> free_events;
+    double hb_ms = 0, or_ms = 0;
+    uint64_t hb_launches = 0, or_launches = 0;
+    char err[512] = {0};
+};
+
+namespace {
+
+const char* kNullHandle = "null lattice handle";
+
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) { cudaSetDevice(dev); switched = true; }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+su_status fail(su_lattice* h, su_status st, const char* fmt, const char* detail = "") {
+    if (h) snprintf(h->err, sizeof(h->err), fmt, detail);
+    return st;
+}
+su_status cuda_fail(su_lattice* h, cudaError_t e, const char* where) {
+    if (h) snprintf(h->err, sizeof(h->err), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+    return SU_ECUDA;
+}
+#define SU_CUDA(h, call, where)                                   \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return cuda_fail(h, e__, where);  \
+    } while (0)
+
+bool dims_ok(int Nc, int Lx, int Ly, int Lz, int Lt) {
+    const int L[4] = {Lx, Ly, Lz, Lt};
+    for (int d = 0; d < 4; ++d) if (L[d] < 2 || (L[d] & 1)) return false;     // reading R7
+    if (Nc < 2) return false;
+    return (double)Lx * Ly * Lz * Lt <= 4294967295.0;   // the site index is one 32-bit RNG counter word
+}
+
+int elems_per_link(int Nc, su_storage s) { return Nc == 2 ? 2 : (s == SU_STORE_RECON12 ? 6 : Nc * Nc); }
+
+#define SU_BY_NC(h, FN, ...)                                                   \
+    ([&]() -> cudaError_t {                                                    \
+        switch ((h)->Nc) {                                                     \
+            case 2: return FN##2(__VA_ARGS__);                                 \
+            case 3: return FN##3(__VA_ARGS__);                                 \
+            case 4: return FN##4(__VA_ARGS__);                                 \
+            case 5: return FN##5(__VA_ARGS__);                                 \
+            case 6: return FN##6(__VA_ARGS__);                                 \
+            case 7: return FN##7(__VA_ARGS__);                                 \
+            case 8: return FN##8(__VA_ARGS__);                                 \
+            default: return cudaErrorInvalidValue;                             \
+        }                                                                      \
+    })()
+
+AuxArgs aux_args(su_lattice* h) {
+    AuxArgs a{};
+    a.links = h->links; a.g = h->g; a.partials = h->d_partials; a.result = h->d_result;
+    a.staging = h->d_staging; a.site0 = 0; a.nsites = 0;
+    a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
+    return a;
+}
+
+__global__ void k_set_u32(uint32_t* p, uint32_t v) { *p = v; }
+
+su_status launch_substep(su_lattice* h, double beta, int kind, int pass, int parity, int mu,
+                         uint8_t* d_attempts, const uint32_t* d_sweep) {
+    UpdateArgs a{};
+    a.links = h->links; a.g = h->g; a.parity = parity; a.mu = mu; a.beta = beta;
+    a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
+    a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = (uint32_t)pass;
+    a.attempts = d_attempts; a.counters = h->d_counters;
+    SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "update kernel launch");
+    return SU_OK;
+}
+
+cudaEvent_t take_event(su_lattice* h) {
+    cudaEvent_t e = nullptr;
+    if (!h->free_events.empty()) { e = h->free_events.back(); h->free_events.pop_back(); }
+    else if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; }
+    return e;
+}
+
+// Fold finished sweeps' event pairs into the per-kind totals (synchronises on the last event).
+void drain_timing(su_lattice* h) {
+    for (auto& s : h->pending) {
+        float a = 0, b = 0;
+        if (cudaEventSynchronize(s.e[2]) == cudaSuccess && cudaEventElapsedTime(&a, s.e[0], s.e[1]) == cudaSuccess &&
+            cudaEventElapsedTime(&b, s.e[1], s.e[2]) == cudaSuccess) {
+            h->hb_ms += a; h->or_ms += b;
+            h->hb_launches += (uint64_t)s.n_hb * 8; h->or_launches += (uint64_t)s.n_or * 8;
+        } else {
+            cudaGetLastError();
+        }
+        for (int i = 0; i < 3; ++i) h->free_events.push_back(s.e[i]);
+    }
+    h->pending.clear();
+}
+
+su_status enqueue_sweep(su_lattice* h, double beta, int n_hb, int n_or, const uint32_t* d_sweep, bool timed) {
+    // reading R6: all heatbath passes, then all overrelaxation passes; parity outer, mu inner
+    su_lattice::SweepEvents ev{};
+    if (timed) {
+        if (h->pending.size() >= 256) drain_timing(h);
+        for (int i = 0; i < 3; ++i) if (!(ev.e[i] = take_event(h))) return fail(h, SU_ECUDA, "cudaEventCreate failed");
+        ev.n_hb = n_hb; ev.n_or = n_or;
+        SU_CUDA(h, cudaEventRecord(ev.e[0], h->stream), "timing event");
+    }
+    for (int pass = 0; pass < n_hb + n_or; ++pass) {
+        const int kind = pass < n_hb ? KIND_HB : KIND_OR;
+        if (timed && pass == n_hb) SU_CUDA(h, cudaEventRecord(ev.e[1], h->stream), "timing event");
+        for (int parity = 0; parity < 2; ++parity)
+            for (int mu = 0; mu < 4; ++mu) {
+                su_status st = launch_substep(h, beta, kind, kind == KIND_HB ? pass : 0, parity, mu, nullptr, d_sweep);
+                if (st != SU_OK) return st;
+            }
+    }
+    if (timed) {
+        if (n_or == 0) SU_CUDA(h, cudaEventRecord(ev.e[1], h->stream), "timing event");
+        SU_CUDA(h, cudaEventRecord(ev.e[2], h->stream), "timing event");
+        h->pending.push_back(ev);
+    }
+    return SU_OK;
+}
+
+su_status ensure_staging(su_lattice* h, size_t bytes) {
+    if (h->staging_bytes >= bytes) return SU_OK;
+    if (h->d_staging) { cudaFree(h->d_staging); h->d_staging = nullptr; h->staging_bytes = 0; }
+    if (cudaMalloc(&h->d_staging, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, SU_ENOMEM, "device staging allocation failed"); }
+    h->staging_bytes = bytes;
+    return SU_OK;
+}
+
+void free_graphs(su_lattice* h) {
+    for (auto& kv : h->graphs) cudaGraphExecDestroy(kv.second);
+    h->graphs.clear();
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t su_lattice_bytes(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, su_storage s) {
+    if (!dims_ok(Nc, Lx, Ly, Lz, Lt) || (p != SU_FP32 && p != SU_FP64)) return 0;
+    if (s != SU_STORE_FULL && s != SU_STORE_RECON12) return 0;
+    if (s == SU_STORE_RECON12 && Nc != 3) return 0;
+    const size_t V = (size_t)Lx * Ly * Lz * Lt;
+    const size_t b = 4 * V * (size_t)elems_per_link(Nc, s) * 2 * (p == SU_FP64 ? 8 : 4);
+    return (b + 255) / 256 * 256;
+}
+
+su_status su_lattice_create(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, su_lattice** out) {
+    return su_lattice_create_ex(Nc, Lx, Ly, Lz, Lt, p, nullptr, out);
+}
+
+su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, const su_options* opt,
+                               su_lattice** out) {
+    if (!out) return SU_EINVAL;
+    su_options o{};
+    o.storage = SU_STORE_FULL; o.kernel = SU_KERNEL_AUTO; o.device = -1;
+    if (opt) o = *opt;
+    if (!dims_ok(Nc, Lx, Ly, Lz, Lt)) return SU_EINVAL;
+    if (p != SU_FP32 && p != SU_FP64) return SU_EINVAL;
+    if (o.storage != SU_STORE_FULL && o.storage != SU_STORE_RECON12) return SU_EINVAL;
+    if (o.storage == SU_STORE_RECON12 && Nc != 3) return SU_EINVAL;
+    if (o.kernel != SU_KERNEL_AUTO && o.kernel != SU_KERNEL_SPECIALISED && o.kernel != SU_KERNEL_GENERIC) return SU_EINVAL;
+    if (Nc > SU_MAX_NC) return SU_EUNSUPPORTED;
+    if (o.kernel == SU_KERNEL_SPECIALISED && Nc > 4) return SU_EUNSUPPORTED;
+
+    su_lattice* h = new (std::nothrow) su_lattice;
+    if (!h) return SU_ENOMEM;
+    h->Nc = Nc;
+    h->g.L[0] = Lx; h->g.L[1] = Ly; h->g.L[2] = Lz; h->g.L[3] = Lt;
+    h->g.Lxh = Lx / 2;
+    h->V = (size_t)Lx * Ly * Lz * Lt;
+    h->g.Vh = (unsigned)(h->V / 2);
+    h->prec = p;
+    h->var.Nc = Nc; h->var.prec = (int)p;
+    h->var.store = Nc == 2 ? STORE_QUAT : (o.storage == SU_STORE_RECON12 ? STORE_RECON12 : STORE_FULL);
+    h->var.generic = (o.kernel == SU_KERNEL_GENERIC) || (o.kernel == SU_KERNEL_AUTO && Nc > 4);
+    h->stream = (cudaStream_t)o.stream;
+
+    cudaError_t e = cudaSuccess;
+    if (o.device < 0) e = cudaGetDevice(&h->device); else h->device = o.device;
+    if (e != cudaSuccess) { delete h; return SU_ECUDA; }
+    DeviceGuard guard(h->device);
+    h->links_bytes = su_lattice_bytes(Nc, Lx, Ly, Lz, Lt, p, o.storage);
+    su_status st = SU_OK;
+    if (o.buffer) {
+        if (o.buffer_bytes < h->links_bytes || ((uintptr_t)o.buffer & 255u)) st = SU_ENOMEM;
+        h->links = o.buffer;
+    } else {
+        if (cudaMalloc(&h->links, h->links_bytes) != cudaSuccess) st = SU_ENOMEM;
+        h->owns_links = (st == SU_OK);
+    }
+    const unsigned Vs = (unsigned)Lx * Ly * Lz;
+    const size_t npart = (size_t)reduce_blocks(2u * h->g.Vh) + 2 * (size_t)reduce_blocks(Vs) + 2;
+    if (st == SU_OK && cudaMalloc(&h->d_partials, npart * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
+    if (st == SU_OK && cudaMalloc(&h->d_result, 2 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
+    if (st == SU_OK && cudaMalloc(&h->d_counters, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ENOMEM;
+    if (st == SU_OK && cudaMalloc(&h->d_sweep, sizeof(uint32_t)) != cudaSuccess) st = SU_ENOMEM;
+    if (st == SU_OK && cudaMemset(h->d_counters, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ECUDA;
+    if (st != SU_OK) { cudaGetLastError(); su_lattice_destroy(h); return st; }
+    *out = h;
+    return SU_OK;
+}
+
+su_status su_lattice_destroy(su_lattice* h) {
+    if (!h) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    cudaStreamSynchronize(h->stream);
+    free_graphs(h);
+    drain_timing(h);
+    for (cudaEvent_t e : h->free_events) cudaEventDestroy(e);
+    if (h->owns_links && h->links) cudaFree(h->links);
+    if (h->d_partials) cudaFree(h->d_partials);
+    if (h->d_result) cudaFree(h->d_result);
+    if (h->d_counters) cudaFree(h->d_counters);
+    if (h->d_sweep) cudaFree(h->d_sweep);
+    if (h->d_attempts) cudaFree(h->d_attempts);
+    if (h->d_staging) cudaFree(h->d_staging);
+    cudaGetLastError();
+    delete h;
+    return SU_OK;
+}
+
+static su_status init_common(su_lattice* h, uint64_t seed, bool hot) {
+    if (!h) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    h->seed = seed; h->sweep = 0;
+    SU_CUDA(h, cudaMemsetAsync(h->d_counters, 0, 2 * sizeof(unsigned long long), h->stream), "counter reset");
+    AuxArgs a = aux_args(h);
+    if (hot) SU_CUDA(h, SU_BY_NC(h, init_hot_nc, h->var, a, h->stream, &h->n_launch), "hot start");
+    else     SU_CUDA(h, SU_BY_NC(h, init_cold_nc, h->var, a, h->stream, &h->n_launch), "cold start");
+    h->ready = true;
+    return SU_OK;
+}
+su_status su_init_cold(su_lattice* h, uint64_t seed) { return init_common(h, seed, false); }
+su_status su_init_hot(su_lattice* h, uint64_t seed) { return init_common(h, seed, true); }
+
+su_status su_set_rng(su_lattice* h, uint64_t seed, uint32_t sweep_counter) {
+    if (!h) return SU_EINVAL;
+    if (seed != h->seed) { DeviceGuard guard(h->device); free_graphs(h); }   // the key is baked into captured launches
+    h->seed = seed; h->sweep = sweep_counter;
+    return SU_OK;
+}
+
+su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
+    if (!h) return SU_EINVAL;
+    if (!(beta >= 0.0) || !std::isfinite(beta) || n_hb < 0 || n_or < 0 || n_hb > 255)
+        return fail(h, SU_EINVAL, "su_sweep: beta must be finite and >= 0, 0 <= n_heatbath <= 255, n_overrelax >= 0");
+    if (!h->ready) return fail(h, SU_ESTATE, "su_sweep before su_init_* / su_import_links");
+    DeviceGuard guard(h->device);
+    if (!h->graph_mode) {
+        su_status st = enqueue_sweep(h, beta, n_hb, n_or, nullptr, h->timing);
+        if (st != SU_OK) return st;
+    } else {
+        // the captured kernels read the sweep counter from device memory, so one graph serves every sweep
+        auto key = std::make_tuple(beta, n_hb, n_or);
+        auto it = h->graphs.find(key);
+        if (it == h->graphs.end()) {
+            cudaStream_t cap;
+            SU_CUDA(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking), "graph capture stream");
+            cudaStream_t user = h->stream;
+            h->stream = cap;
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+            su_status st = SU_OK;
+            const uint64_t before = h->n_launch;
+            if (e == cudaSuccess) st = enqueue_sweep(h, beta, n_hb, n_or, h->d_sweep, false);
+            if (e == cudaSuccess) e = cudaStreamEndCapture(cap, &graph);
+            h->n_launch = before;
+            h->stream = user;
+            cudaGraphExec_t exec = nullptr;
+            if (e == cudaSuccess && st == SU_OK) e = cudaGraphInstantiate(&exec, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+            cudaStreamDestroy(cap);
+            if (st != SU_OK) return st;
+            if (e != cudaSuccess) return cuda_fail(h, e, "graph capture");
+            it = h->graphs.emplace(key, exec).first;
+        }
+        k_set_u32<<<1, 1, 0, h->stream>>>(h->d_sweep, h->sweep);
+        SU_CUDA(h, cudaGetLastError(), "sweep counter upload");
+        SU_CUDA(h, cudaGraphLaunch(it->second, h->stream), "graph launch");
+        h->n_launch += 1 + (uint64_t)(n_hb + n_or) * 8;
+    }
+    ++h->sweep;
+    return SU_OK;
+}
+
+su_status su_substep(su_lattice* h, double beta, int kind, int pass, int parity, int mu, uint8_t* host_attempts) {
+    if (!h) return SU_EINVAL;
+    if (!(beta >= 0.0) || !std::isfinite(beta) || kind < 0 || kind > 1 || pass < 0 || pass > 255 || parity < 0 ||
+        parity > 1 || mu < 0 || mu > 3)
+        return fail(h, SU_EINVAL, "su_substep: argument out of range");
+    if (!h->ready) return fail(h, SU_ESTATE, "su_substep before su_init_* / su_import_links");
+    DeviceGuard guard(h->device);
+    const size_t nsub = (size_t)h->Nc * (h->Nc - 1) / 2, nbytes = nsub * h->g.Vh;
+    if (host_attempts) {
+        if (!h->d_attempts && cudaMalloc(&h->d_attempts, nbytes) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(h, SU_ENOMEM, "attempt buffer allocation failed");
+        }
+        SU_CUDA(h, cudaMemsetAsync(h->d_attempts, 0, nbytes, h->stream), "attempt buffer reset");
+    }
+    su_status st = launch_substep(h, beta, kind, pass, parity, mu, host_attempts ? h->d_attempts : nullptr, nullptr);
+    if (st != SU_OK) return st;
+    if (host_attempts) {
+        SU_CUDA(h, cudaMemcpyAsync(host_attempts, h->d_attempts, nbytes, cudaMemcpyDeviceToHost, h->stream), "attempt copy");
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_substep synchronise");
+    }
+    return SU_OK;
+}
+
+su_status su_plaquette(su_lattice* h, double* out) {
+    if (!h || !out) return SU_EINVAL;
+    if (!h->ready) return fail(h, SU_ESTATE, "su_plaquette before su_init_* / su_import_links");
+    DeviceGuard guard(h->device);
+    AuxArgs a = aux_args(h);
+    SU_CUDA(h, SU_BY_NC(h, plaquette_nc, h->var, a, h->stream, &h->n_launch), "plaquette kernels");
+    double v = 0;
+    SU_CUDA(h, cudaMemcpyAsync(&v, h->d_result, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "plaquette copy");
+    SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_plaquette synchronise");
+    *out = v;
+    return SU_OK;
+}
+
+su_status su_polyakov(su_lattice* h, double out[2]) {
+    if (!h || !out) return SU_EINVAL;
+    if (!h->ready) return fail(h, SU_ESTATE, "su_polyakov before su_init_* / su_import_links");
+    DeviceGuard guard(h->device);
+    AuxArgs a = aux_args(h);
+    SU_CUDA(h, SU_BY_NC(h, polyakov_nc, h->var, a, h->stream, &h->n_launch), "polyakov kernels");
+    double v[2] = {0, 0};
+    SU_CUDA(h, cudaMemcpyAsync(v, h->d_result, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream), "polyakov copy");
+    SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_polyakov synchronise");
+    out[0] = v[0]; out[1] = v[1];
+    return SU_OK;
+}
+
+su_status su_reunitarize(su_lattice* h) {
+    if (!h) return SU_EINVAL;
+    if (!h->ready) return fail(h, SU_ESTATE, "su_reunitarize before su_init_* / su_import_links");
+    DeviceGuard guard(h->device);
+    AuxArgs a = aux_args(h);
+    SU_CUDA(h, SU_BY_NC(h, reunit_nc, h->var, a, h->stream, &h->n_launch), "reunitarise kernel");
+    return SU_OK;
+}
+
+static su_status transfer_links(su_lattice* h, double* host, size_t n_doubles, bool to_host) {
+    const size_t per_site = 4 * 2 * (size_t)h->Nc * h->Nc;                  // doubles per site
+    if (n_doubles != h->V * per_site) return fail(h, SU_EINVAL, "link array size must be 4 V * 2 Nc^2 doubles");
+    DeviceGuard guard(h->device);
+    const size_t chunk_sites_max = (size_t)(64u << 20) / (per_site * sizeof(double)) + 1;
+    const size_t chunk_sites = chunk_sites_max < h->V ? chunk_sites_max : h->V;
+    su_status st = ensure_staging(h, chunk_sites * per_site * sizeof(double));
+    if (st != SU_OK) return st;
+    for (size_t s0 = 0; s0 < h->V; s0 += chunk_sites) {
+        const size_t ns = (h->V - s0 < chunk_sites) ? h->V - s0 : chunk_sites;
+        AuxArgs a = aux_args(h);
+        a.site0 = (unsigned)s0; a.nsites = (unsigned)ns;
+        double* hp = host + s0 * per_site;
+        if (to_host) {
+            SU_CUDA(h, SU_BY_NC(h, export_nc, h->var, a, h->stream, &h->n_launch), "export kernel");
+            SU_CUDA(h, cudaMemcpyAsync(hp, h->d_staging, ns * per_site * sizeof(double), cudaMemcpyDeviceToHost, h->stream), "export copy");
+        } else {
+            SU_CUDA(h, cudaMemcpyAsync(h->d_staging, hp, ns * per_site * sizeof(double), cudaMemcpyHostToDevice, h->stream), "import copy");
+            SU_CUDA(h, SU_BY_NC(h, import_nc, h->var, a, h->stream, &h->n_launch), "import kernel");
+        }
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "link transfer synchronise");
+    }
+    return SU_OK;
+}
+
+su_status su_export_links(su_lattice* h, double* host_dst, size_t n_doubles) {
+    if (!h || !host_dst) return SU_EINVAL;
+    if (!h->ready) return fail(h, SU_ESTATE, "su_export_links before su_init_* / su_import_links");
+    return transfer_links(h, host_dst, n_doubles, true);
+}
+
+su_status su_import_links(su_lattice* h, const double* host_src, size_t n_doubles) {
+    if (!h || !host_src) return SU_EINVAL;
+    su_status st = transfer_links(h, const_cast<double*>(host_src), n_doubles, false);
+    if (st == SU_OK) h->ready = true;
+    return st;
+}
+
+su_status su_get_counters(su_lattice* h, uint64_t* kp_attempts_total, uint64_t* kp_exhausted) {
+    if (!h) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    unsigned long long v[2] = {0, 0};
+    SU_CUDA(h, cudaMemcpyAsync(v, h->d_counters, sizeof(v), cudaMemcpyDeviceToHost, h->stream), "counter copy");
+    SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_get_counters synchronise");
+    if (kp_attempts_total) *kp_attempts_total = v[0];
+    if (kp_exhausted) *kp_exhausted = v[1];
+    return SU_OK;
+}
+
+su_status su_synchronize(su_lattice* h) {
+    if (!h) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_synchronize");
+    return SU_OK;
+}
+
+su_status su_set_graph_mode(su_lattice* h, int enabled) {
+    if (!h) return SU_EINVAL;
+    h->graph_mode = enabled != 0;
+    return SU_OK;
+}
+
+su_status su_set_timing(su_lattice* h, int enabled) {
+    if (!h) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    drain_timing(h);
+    h->timing = enabled != 0;
+    h->hb_ms = h->or_ms = 0; h->hb_launches = h->or_launches = 0;
+    return SU_OK;
+}
+
+su_status su_get_timing(su_lattice* h, double* hb_ms, uint64_t* hb_launches, double* or_ms, uint64_t* or_launches) {
+    if (!h) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    drain_timing(h);
+    if (hb_ms) *hb_ms = h->hb_ms;
+    if (or_ms) *or_ms = h->or_ms;
+    if (hb_launches) *hb_launches = h->hb_launches;
+    if (or_launches) *or_launches = h->or_launches;
+    return SU_OK;
+}
+
+su_status su_get_launch_count(su_lattice* h, uint64_t* out) {
+    if (!h || !out) return SU_EINVAL;
+    *out = h->n_launch;
+    return SU_OK;
+}
+
+const char* su_last_error(const su_lattice* h) { return h ? h->err : kNullHandle; }
+
+}  // extern "C"

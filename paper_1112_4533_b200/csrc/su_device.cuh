@@ -1,0 +1,350 @@
+// su_device.cuh — device-side building blocks of libsugauge (sm_100a).
+// Complex Nc x Nc arithmetic in registers (UNR=true) or local arrays (UNR=false, generic kernel),
+// checkerboard geometry, SoA link I/O, Philox4x32-10 and the Kennedy-Pendleton draw.
+// Method: Cardoso & Bicudo, arXiv:1112.4533 (PAPER.md cited by line); readings R1..R20 in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sug {
+
+enum : int { STORE_FULL = 0, STORE_RECON12 = 1, STORE_QUAT = 2 };
+enum : int { KIND_HB = 0, KIND_OR = 1 };
+enum : int { RNG_KP = 0, RNG_DIR = 1, RNG_HOT = 2 };
+constexpr int KP_MAX_ATTEMPTS = 1024;   // reading R15
+
+template <class T> struct V2;
+template <> struct V2<float>  { typedef float2  type; static __device__ __forceinline__ float2  make(float a, float b)   { return make_float2(a, b); } };
+template <> struct V2<double> { typedef double2 type; static __device__ __forceinline__ double2 make(double a, double b) { return make_double2(a, b); } };
+
+template <class T> struct cx { T re, im; };
+
+template <class T> __device__ __forceinline__ cx<T> mk(T r, T i) { cx<T> c; c.re = r; c.im = i; return c; }
+template <class T> __device__ __forceinline__ cx<T> conj(cx<T> a) { return mk<T>(a.re, -a.im); }
+template <class T> __device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.re + b.re, a.im + b.im); }
+template <class T> __device__ __forceinline__ cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.re - b.re, a.im - b.im); }
+template <class T> __device__ __forceinline__ cx<T> operator*(cx<T> a, cx<T> b) { return mk<T>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re); }
+template <class T> __device__ __forceinline__ cx<T> operator*(T s, cx<T> a) { return mk<T>(s * a.re, s * a.im); }
+// acc += a b ; acc += a conj(b) ; acc += conj(a) b
+template <class T> __device__ __forceinline__ void mad(cx<T>& acc, cx<T> a, cx<T> b) {
+    acc.re += a.re * b.re; acc.re -= a.im * b.im; acc.im += a.re * b.im; acc.im += a.im * b.re;
+}
+template <class T> __device__ __forceinline__ void mad_cb(cx<T>& acc, cx<T> a, cx<T> b) {
+    acc.re += a.re * b.re; acc.re += a.im * b.im; acc.im += a.im * b.re; acc.im -= a.re * b.im;
+}
+template <class T> __device__ __forceinline__ void mad_ca(cx<T>& acc, cx<T> a, cx<T> b) {
+    acc.re += a.re * b.re; acc.re += a.im * b.im; acc.im += a.re * b.im; acc.im -= a.im * b.re;
+}
+
+// ------------------------------------------------------------------------------------------
+// Geometry (readings R7): even extents, periodic, checkerboard index cb = i/2.
+// ------------------------------------------------------------------------------------------
+struct Geom {
+    int L[4];
+    int Lxh;        // Lx / 2
+    unsigned Vh;    // V / 2 = sites per parity
+};
+
+__device__ __forceinline__ void decode_cb(const Geom& g, unsigned cb, int parity, int c[4]) {
+    unsigned xh = cb % (unsigned)g.Lxh, r = cb / (unsigned)g.Lxh;
+    c[1] = (int)(r % (unsigned)g.L[1]); r /= (unsigned)g.L[1];
+    c[2] = (int)(r % (unsigned)g.L[2]);
+    c[3] = (int)(r / (unsigned)g.L[2]);
+    c[0] = 2 * (int)xh + ((c[1] + c[2] + c[3] + parity) & 1);
+}
+__device__ __forceinline__ unsigned cb_of(const Geom& g, int x, int y, int z, int t) {
+    return (unsigned)(x >> 1) + (unsigned)g.Lxh * ((unsigned)y + (unsigned)g.L[1] * ((unsigned)z + (unsigned)g.L[2] * (unsigned)t));
+}
+__device__ __forceinline__ unsigned lex_of(const Geom& g, const int c[4]) {
+    return (unsigned)c[0] + (unsigned)g.L[0] * ((unsigned)c[1] + (unsigned)g.L[1] * ((unsigned)c[2] + (unsigned)g.L[2] * (unsigned)c[3]));
+}
+// checkerboard index of c + s1*e_{d1} + s2*e_{d2} (s in {-1,0,+1}), periodic wrap
+__device__ __forceinline__ unsigned cb_shift(const Geom& g, const int c[4], int d1, int s1, int d2 = 0, int s2 = 0) {
+    int n[4] = {c[0], c[1], c[2], c[3]};
+    n[d1] += s1; if (n[d1] < 0) n[d1] += g.L[d1]; if (n[d1] >= g.L[d1]) n[d1] -= g.L[d1];
+    n[d2] += s2; if (n[d2] < 0) n[d2] += g.L[d2]; if (n[d2] >= g.L[d2]) n[d2] -= g.L[d2];
+    return cb_of(g, n[0], n[1], n[2], n[3]);
+}
+
+// ------------------------------------------------------------------------------------------
+// Link I/O on the SoA layout links[mu][parity][elem][cb] of (re,im) pairs.
+// ------------------------------------------------------------------------------------------
+template <int NC, int STORE> struct LinkElems {
+    static constexpr int E = (STORE == STORE_QUAT) ? 2 : ((STORE == STORE_RECON12) ? 6 : NC * NC);
+};
+
+template <class T> __device__ __forceinline__ void su3_third_row(cx<T>* m) {
+    m[6] = conj(m[1] * m[5] - m[2] * m[4]);
+    m[7] = conj(m[2] * m[3] - m[0] * m[5]);
+    m[8] = conj(m[0] * m[4] - m[1] * m[3]);
+}
+
+template <int NC, class T, int STORE, bool UNR> struct LinkIO {
+    typedef typename V2<T>::type T2;
+    static constexpr int E = LinkElems<NC, STORE>::E;
+    static_assert(STORE != STORE_QUAT || NC == 2, "quaternion storage is SU(2) only");
+    static_assert(STORE != STORE_RECON12 || NC == 3, "two-row storage is SU(3) only");
+
+    static __device__ __forceinline__ const T2* plane(const void* base, const Geom& g, int mu, int par) {
+        return (const T2*)base + (size_t)(mu * 2 + par) * E * g.Vh;
+    }
+    static __device__ __forceinline__ T2* plane(void* base, const Geom& g, int mu, int par) {
+        return (T2*)base + (size_t)(mu * 2 + par) * E * g.Vh;
+    }
+    template <bool RO>
+    static __device__ __forceinline__ void load(const T2* __restrict__ pl, unsigned Vh, unsigned cb, cx<T>* m) {
+        if (STORE == STORE_QUAT) {
+            T2 v0 = RO ? __ldg(pl + cb) : pl[cb];
+            T2 v1 = RO ? __ldg(pl + Vh + cb) : pl[Vh + cb];
+            // eq 6: [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]], v0 = (a0,a1), v1 = (a2,a3)
+            m[0] = mk<T>(v0.x, v1.y);  m[1] = mk<T>(v1.x, v0.y);
+            m[2] = mk<T>(-v1.x, v0.y); m[3] = mk<T>(v0.x, -v1.y);
+        } else {
+#pragma unroll(UNR ? E : 1)
+            for (int e = 0; e < E; ++e) {
+                T2 v = RO ? __ldg(pl + (size_t)e * Vh + cb) : pl[(size_t)e * Vh + cb];
+                m[e] = mk<T>(v.x, v.y);
+            }
+            if (STORE == STORE_RECON12) su3_third_row(m);
+        }
+    }
+    static __device__ __forceinline__ void store(T2* __restrict__ pl, unsigned Vh, unsigned cb, const cx<T>* m) {
+        if (STORE == STORE_QUAT) {
+            pl[cb]      = V2<T>::make(m[0].re, m[1].im);
+            pl[Vh + cb] = V2<T>::make(m[1].re, m[0].im);
+        } else {
+#pragma unroll(UNR ? E : 1)
+            for (int e = 0; e < E; ++e) pl[(size_t)e * Vh + cb] = V2<T>::make(m[e].re, m[e].im);
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// Nc x Nc complex products, row-major. UNR: full unroll (registers) or rolled loops (local arrays).
+// ------------------------------------------------------------------------------------------
+template <int NC, class T, bool UNR> struct Mat {
+    typedef cx<T> C;
+    // O = A B
+    static __device__ __forceinline__ void mul_nn(const C* A, const C* B, C* O) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i)
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad(s, A[i * NC + k], B[k * NC + j]);
+                O[i * NC + j] = s;
+            }
+    }
+    // O = A^dagger B
+    static __device__ __forceinline__ void mul_dn(const C* A, const C* B, C* O) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i)
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad_ca(s, A[k * NC + i], B[k * NC + j]);
+                O[i * NC + j] = s;
+            }
+    }
+    // O = A B^dagger
+    static __device__ __forceinline__ void mul_nd(const C* A, const C* B, C* O) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i)
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad_cb(s, A[i * NC + k], B[j * NC + k]);
+                O[i * NC + j] = s;
+            }
+    }
+    // S += A B
+    static __device__ __forceinline__ void acc_nn(C* S, const C* A, const C* B) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i)
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = S[i * NC + j];
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad(s, A[i * NC + k], B[k * NC + j]);
+                S[i * NC + j] = s;
+            }
+    }
+    // S += A B^dagger
+    static __device__ __forceinline__ void acc_nd(C* S, const C* A, const C* B) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i)
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = S[i * NC + j];
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad_cb(s, A[i * NC + k], B[j * NC + k]);
+                S[i * NC + j] = s;
+            }
+    }
+    // Re Tr (A B^dagger) = sum_ij Re(A_ij conj(B_ij))
+    static __device__ __forceinline__ T retr_nd(const C* A, const C* B) {
+        T s = 0;
+#pragma unroll(UNR ? NC * NC : 1)
+        for (int e = 0; e < NC * NC; ++e) s += A[e].re * B[e].re + A[e].im * B[e].im;
+        return s;
+    }
+    static __device__ __forceinline__ void zero(C* S) {
+#pragma unroll(UNR ? NC * NC : 1)
+        for (int e = 0; e < NC * NC; ++e) S[e] = mk<T>(0, 0);
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11): counter (c0..c3), key (k0,k1), 10 rounds.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// uniform in (0,1], exact in T: fp64 (w+1)/2^32, fp32 ((w>>8)+1)/2^24
+template <class T> __device__ __forceinline__ T uniform01(uint32_t w);
+template <> __device__ __forceinline__ double uniform01<double>(uint32_t w) { return ((double)w + 1.0) * (1.0 / 4294967296.0); }
+template <> __device__ __forceinline__ float  uniform01<float >(uint32_t w) { return ((float)(w >> 8) + 1.0f) * (1.0f / 16777216.0f); }
+
+__device__ __forceinline__ uint32_t pack_c2(int kind, int pass, int parity, int mu, int subgroup) {
+    return ((uint32_t)kind << 28) | ((uint32_t)(pass & 0xff) << 20) | ((uint32_t)parity << 19) |
+           ((uint32_t)mu << 17) | (uint32_t)subgroup;
+}
+
+template <class T> struct Fn;
+template <> struct Fn<float> {
+    static __device__ __forceinline__ float log(float x) { return logf(x); }
+    static __device__ __forceinline__ float cos(float x) { return cosf(x); }
+    static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
+    static __device__ __forceinline__ void sincos(float x, float* s, float* c) { sincosf(x, s, c); }
+    static __device__ __forceinline__ float max0(float x) { return fmaxf(x, 0.0f); }
+    static __device__ __forceinline__ bool finite(float x) { return isfinite(x); }
+};
+template <> struct Fn<double> {
+    static __device__ __forceinline__ double log(double x) { return ::log(x); }
+    static __device__ __forceinline__ double cos(double x) { return ::cos(x); }
+    static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+    static __device__ __forceinline__ void sincos(double x, double* s, double* c) { ::sincos(x, s, c); }
+    static __device__ __forceinline__ double max0(double x) { return fmax(x, 0.0); }
+    static __device__ __forceinline__ bool finite(double x) { return isfinite(x); }
+};
+
+// Kennedy-Pendleton draw of v = (a0, a): P(a0) ~ sqrt(1-a0^2) exp(alpha a0) (eq 13),
+// a uniform on the sphere of radius sqrt(1-a0^2). Returns attempts used, 0 = none.
+template <class T>
+__device__ __forceinline__ int kp_draw(T alpha, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
+                                       uint32_t c2_base, T v[4]) {
+    const T TWO_PI = (T)6.283185307179586476925286766559;
+    if (!(alpha > (T)0) || !Fn<T>::finite(alpha)) return 0;
+    const T inv2a = (T)2 * alpha;
+    T a0 = 0;
+    int used = 0;
+    for (int n = 0; n < KP_MAX_ATTEMPTS; ++n) {
+        uint32_t w[4];
+        philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_KP << 28), (uint32_t)n, k0, k1, w);
+        T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]), r4 = uniform01<T>(w[3]);
+        T c = Fn<T>::cos(TWO_PI * r2);
+        T lambda2 = -(Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) / inv2a;
+        if (r4 * r4 <= (T)1 - lambda2) { a0 = (T)1 - (T)2 * lambda2; used = n + 1; break; }
+    }
+    if (!used) return 0;
+    uint32_t w[4];
+    philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_DIR << 28), 0u, k0, k1, w);
+    T u1 = uniform01<T>(w[0]), u2 = uniform01<T>(w[1]);
+    T cos_t = (T)1 - (T)2 * u1;
+    T sin_t = Fn<T>::sqrt(Fn<T>::max0((T)1 - cos_t * cos_t));
+    T rho = Fn<T>::sqrt(Fn<T>::max0((T)1 - a0 * a0));
+    T sp, cp;
+    Fn<T>::sincos(TWO_PI * u2, &sp, &cp);
+    v[0] = a0; v[1] = rho * sin_t * cp; v[2] = rho * sin_t * sp; v[3] = rho * cos_t;
+    return used;
+}
+
+// quaternion product, U = a0 + i a.sigma (eq 6): (ab)_0 = a0 b0 - a.b, (ab)_vec = a0 b + b0 a - a x b
+template <class T> __device__ __forceinline__ void quat_mul(const T a[4], const T b[4], T o[4]) {
+    o[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
+    o[1] = a[0] * b[1] + b[0] * a[1] - (a[2] * b[3] - a[3] * b[2]);
+    o[2] = a[0] * b[2] + b[0] * a[2] - (a[3] * b[1] - a[1] * b[3]);
+    o[3] = a[0] * b[3] + b[0] * a[3] - (a[1] * b[2] - a[2] * b[1]);
+}
+
+// ------------------------------------------------------------------------------------------
+// Steps 3-5 of the Cabibbo-Marinari procedure on one link (eqs 11-17): every
+// SU(2) subgroup (i<j), lexicographic (reading R5): project the 2x2 block of W, heatbath
+// (alpha = 2 beta k / Nc, reading R3) or overrelaxation, left-multiply rows i,j of U and W (eq 15).
+// att: attempts per subgroup (NULL ok). Returns (attempts_total, exhausted) packed: lo 24 bits / hi 8.
+// ------------------------------------------------------------------------------------------
+template <int NC, class T, int KIND, bool UNR>
+__device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uint32_t k0, uint32_t k1,
+                                                 uint32_t c0, uint32_t c1, uint32_t c2_base,
+                                                 uint8_t* att_out, size_t att_stride,
+                                                 unsigned& att_total, unsigned& exhausted) {
+    int q = 0;
+#pragma unroll(UNR ? NC : 1)
+    for (int i = 0; i < NC - 1; ++i) {
+#pragma unroll(UNR ? NC : 1)
+        for (int j = i + 1; j < NC; ++j, ++q) {
+            const cx<T> wii = W[i * NC + i], wij = W[i * NC + j], wji = W[j * NC + i], wjj = W[j * NC + j];
+            T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
+            T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
+            T k = Fn<T>::sqrt(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
+            bool ok = (k > (T)0) && Fn<T>::finite(k);
+            T a[4] = {(T)1, (T)0, (T)0, (T)0};
+            int used = 0;
+            if (ok) {
+                T ud[4] = {r0 / k, -r1 / k, -r2 / k, -r3 / k};
+                if (KIND == KIND_HB) {
+                    T v[4];
+                    used = kp_draw<T>((T)2 * beta * k / (T)NC, k0, k1, c0, c1, c2_base | (uint32_t)q, v);
+                    if (used) quat_mul(v, ud, a); else ok = false;
+                } else {
+                    quat_mul(ud, ud, a);
+                }
+            }
+            if (KIND == KIND_HB) {
+                att_total += (unsigned)used;
+                if (!ok) exhausted += 1u;
+                if (att_out) att_out[(size_t)q * att_stride] = (uint8_t)(used > 255 ? 255 : used);
+            }
+            if (ok) {
+                const cx<T> a00 = mk<T>(a[0], a[3]), a01 = mk<T>(a[2], a[1]);
+                const cx<T> a10 = mk<T>(-a[2], a[1]), a11 = mk<T>(a[0], -a[3]);
+#pragma unroll(UNR ? NC : 1)
+                for (int c = 0; c < NC; ++c) {
+                    cx<T> ui = U[i * NC + c], uj = U[j * NC + c];
+                    U[i * NC + c] = a00 * ui + a01 * uj;
+                    U[j * NC + c] = a10 * ui + a11 * uj;
+                    cx<T> wi = W[i * NC + c], wj = W[j * NC + c];
+                    W[i * NC + c] = a00 * wi + a01 * wj;
+                    W[j * NC + c] = a10 * wi + a11 * wj;
+                }
+            }
+        }
+    }
+}
+
+// block-wide sum of doubles (warp shuffle, then shared memory across warps); result in thread 0
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sh[32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (lane == 0) sh[w] = v;
+    __syncthreads();
+    v = (threadIdx.x < nw) ? sh[threadIdx.x] : 0.0;
+    if (w == 0) for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+}  // namespace sug

@@ -1,0 +1,61 @@
+// su_internal.h — host-side declarations shared by the translation units of libsugauge.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/su_gauge.h"
+#include "su_device.cuh"
+
+namespace sug {
+
+struct UpdateArgs {
+    void* links;
+    Geom g;
+    int parity, mu;
+    double beta;
+    uint32_t k0, k1, sweep, pass;
+    const uint32_t* sweep_ptr;         // device; when non-NULL the sweep counter is read from here (graph replay)
+    uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
+    unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
+};
+
+struct Variant {
+    int Nc;
+    int prec;      // su_precision
+    int store;     // STORE_FULL / STORE_RECON12 / STORE_QUAT
+    bool generic;  // rolled-loop generic kernel instead of the register-resident one
+};
+
+struct AuxArgs {
+    void* links;
+    Geom g;
+    double* partials;        // device scratch for reductions
+    double* result;          // device, up to 2 doubles
+    double* staging;         // device, canonical layout chunk
+    unsigned site0, nsites;  // lexicographic site range for import/export
+    uint32_t k0, k1;
+};
+
+// Each returns cudaGetLastError() after the launch; n_launch is incremented per kernel launched.
+#define SUG_DECLARE_NC(N)                                                                                   \
+    cudaError_t update_nc##N(const Variant&, int kind, const UpdateArgs&, cudaStream_t, uint64_t* n_launch); \
+    cudaError_t plaquette_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);           \
+    cudaError_t polyakov_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);            \
+    cudaError_t reunit_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);              \
+    cudaError_t init_cold_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);           \
+    cudaError_t init_hot_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);            \
+    cudaError_t export_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);              \
+    cudaError_t import_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+
+SUG_DECLARE_NC(2)
+SUG_DECLARE_NC(3)
+SUG_DECLARE_NC(4)
+SUG_DECLARE_NC(5)
+SUG_DECLARE_NC(6)
+SUG_DECLARE_NC(7)
+SUG_DECLARE_NC(8)
+
+constexpr int REDUCE_BLOCK = 256;
+inline unsigned reduce_blocks(unsigned n) { return (n + REDUCE_BLOCK - 1) / REDUCE_BLOCK; }
+
+}  // namespace sug
