@@ -79,3 +79,339 @@ def ncu_traffic(tag):
         return json.load(open(p)).get(tag)
     except Exception:
         return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200", "-i", str(gpu_index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        inside = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows]
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in inside:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_lattice(su, wl, precision, recon12, kernel, rank, device):
+    lat = su.Lattice(wl["Nc"], (wl["L"],) * 4, precision, recon12=recon12, kernel=kernel, device=device)
+    if wl["start"] == "hot":
+        lat.init_hot(wl["seed"] + rank)
+    else:
+        lat.init_cold(wl["seed"] + rank)
+    return lat
+
+
+def one_step(lat, beta, reunit):
+    """the whole hot path once: 40 update kernels + reunitarise + both reductions (24 bytes D2H)"""
+    lat.sweep(beta, N_HB, N_OR)
+    if reunit:
+        lat.reunitarize()
+    return lat.plaquette(), lat.polyakov()
+
+
+def time_resident(torch, dist, lat, wl, steps, warmup, sample_clocks, gpu_index):
+    """K steps with the lattice resident in HBM; CUDA events on the launching stream; max over ranks."""
+    reunit = wl["Nc"] > 2
+    for _ in range(warmup):
+        one_step(lat, wl["beta"], reunit)
+    lat.set_timing(True)
+    n0 = lat.launch_count()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(gpu_index) if sample_clocks else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    ev0.record(lat.stream)
+    for _ in range(steps):
+        plaq, poly = one_step(lat, wl["beta"], reunit)
+    ev1.record(lat.stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    if dist is not None:
+        dist.barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop(t0, t1) if sampler else None
+    tim = lat.timing()
+    lat.set_timing(False)
+    launches = lat.launch_count() - n0
+    att, exh = lat.counters()
+    return dict(ms=ms, wall_ms=(t1 - t0) * 1e3, clocks=clocks, timing=tim, launches=launches, plaquette=plaq,
+                polyakov=[poly.real, poly.imag], kp_exhausted=exh)
+
+
+def time_e2e(torch, dist, lat, wl, steps):
+    """Same step through the C ABI with HOST buffers: every step copies the configuration in from pinned
+    host memory (su_import_links, canonical doubles), runs the hot path, and copies the new configuration
+    back out (su_export_links) plus the 24 bytes of observables."""
+    import numpy as np
+    reunit = wl["Nc"] > 2
+    n_doubles = 4 * lat.V * 2 * lat.Nc * lat.Nc
+    pinned = torch.empty(n_doubles, dtype=torch.float64, pin_memory=True)
+    host = pinned.numpy().view(np.complex128).reshape(lat.dims[::-1] + (4, lat.Nc, lat.Nc))
+    lat.export_links(out=host)
+    for _ in range(1):
+        lat.import_links(host); one_step(lat, wl["beta"], reunit); lat.export_links(out=host)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    ev0.record(lat.stream)
+    for _ in range(steps):
+        lat.import_links(host)
+        one_step(lat, wl["beta"], reunit)
+        lat.export_links(out=host)
+    ev1.record(lat.stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    if dist is not None:
+        dist.barrier()
+    ms = max(ev0.elapsed_time(ev1), (t1 - t0) * 1e3)       # host-side copies count: take the longer clock
+    return dict(ms=ms, steps=steps, h2d=n_doubles * 8, d2h=n_doubles * 8 + 24)
+
+
+# ---- the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference) -----------------------
+def oracle_substep_rate(wl, precision, recon12, L, budget_s):
+    """Time oracle sub-steps of the 1 HB + 4 OR schedule on an L^4 lattice with the workload's group,
+    coupling and start; returns (link updates/s over a 1+4 mix, threads, description, seconds spent)."""
+    import oracle
+    t_start = time.perf_counter()
+    O = oracle.OracleLattice(wl["Nc"], (L,) * 4, precision, recon12)
+    (O.init_hot if wl["start"] == "hot" else O.init_cold)(wl["seed"])
+    half = O.V // 2
+    t_kind = {}
+    for kind in (0, 1):
+        n, t = 0, 0.0
+        while n < 8 and (n == 0 or t < budget_s / 2):
+            t0 = time.perf_counter()
+            O.substep(wl["beta"], kind, 0, n // 4 % 2, n % 4)
+            t += time.perf_counter() - t0
+            n += 1
+        t_kind[kind] = (t / n, n)
+    t_mix = N_HB * t_kind[0][0] + N_OR * t_kind[1][0]            # per (parity, mu): 1 HB + 4 OR sub-steps
+    rate = (N_HB + N_OR) * half / t_mix
+    desc = (f"SU({wl['Nc']}) {L}^4 {precision}{' recon12' if recon12 else ''} beta {wl['beta']} {wl['start']} start: "
+            f"{t_kind[0][1]} heatbath + {t_kind[1][1]} overrelaxation sub-steps ({half} link updates each), "
+            f"combined 1:4 as in the sweep")
+    threads = oracle.num_threads()
+    O.close()
+    return rate, threads, desc, time.perf_counter() - t_start
+
+
+def cpu_baseline(wl, precision, recon12, budget_s=20.0):
+    import oracle
+    # probe on 8^4 to pick the largest lattice (<= the workload's) whose sub-steps fit the budget
+    r0, threads, _, _ = oracle_substep_rate(wl, precision, recon12, 8, 0.5)
+    L = wl["L"]
+    while L > 8 and (L ** 4 / 2) * 10 / r0 > budget_s * 3:        # ~10 sub-steps + init
+        L = {48: 32, 32: 24, 24: 16, 16: 12, 12: 8}.get(L, 8)
+    rate, threads, desc, spent = oracle_substep_rate(wl, precision, recon12, L, budget_s)
+    return {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+            "host_cpus": os.cpu_count(), "seconds": round(spent, 2)}
+
+
+def run_reference(args, wl, rank):
+    """--impl reference: the oracle on the host cores, one bounded sample (sub-steps of the sweep) per step."""
+    if rank != 0:
+        return 0
+    import oracle
+    precision, recon12 = args.precision, args.storage == "recon12"
+    r0, threads, _, _ = oracle_substep_rate(wl, precision, recon12, 8, 0.5)
+    budget_step = 150.0 / max(1, args.steps + args.warmup)
+    L = wl["L"]
+    while L > 8 and (L ** 4 / 2) / r0 > budget_step:
+        L = {48: 32, 32: 24, 24: 16, 16: 12, 12: 8}.get(L, 8)
+    O = oracle.OracleLattice(wl["Nc"], (L,) * 4, precision, recon12)
+    (O.init_hot if wl["start"] == "hot" else O.init_cold)(wl["seed"])
+    half = O.V // 2
+    sched = [(0 if p < N_HB else 1, parity, mu) for p in range(N_HB + N_OR) for parity in range(2) for mu in range(4)]
+    i = 0
+    for _ in range(args.warmup):
+        kind, parity, mu = sched[i % 40]; O.substep(wl["beta"], kind, 0, parity, mu); i += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        kind, parity, mu = sched[i % 40]; O.substep(wl["beta"], kind, 0, parity, mu); i += 1
+    dt = time.perf_counter() - t0
+    value = args.steps * half / dt
+    sample = (f"SU({wl['Nc']}) {L}^4 {precision} beta {wl['beta']} {wl['start']} start; each step = one (parity, mu) "
+              f"sub-step of the 1 HB + 4 OR schedule ({half} link updates), schedule order, on {threads} OpenMP threads")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64" if precision == "fp64" else "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "Nc": wl["Nc"], "lattice": f"{wl['L']}^4", "beta": wl["beta"],
+                       "sweep": "1 heatbath + 4 overrelaxation", "storage": args.storage, "sample_lattice": f"{L}^4"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
+    """Turn one timed run into the metric, GFLOPS and the roofline object of its dominant (OR) kernel."""
+    Nc, V = wl["Nc"], wl["L"] ** 4
+    updates_step = (N_HB + N_OR) * 4 * V
+    t_step = res["ms"] / steps * 1e-3
+    value = n_ranks * updates_step / t_step
+    flops_step = 4 * V * (N_HB * flops_per_update(Nc, "hb", recon12) + N_OR * flops_per_update(Nc, "or", recon12))
+    bpu = algorithmic_bytes_per_update(Nc, precision, recon12)
+    tim = res["timing"]
+    roof = None
+    if tim["or_launches"]:
+        or_ms = tim["or_ms"] / tim["or_launches"]
+        hb_ms = tim["hb_ms"] / tim["hb_launches"] if tim["hb_launches"] else None
+        ach = bpu * (V // 2) / (or_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_update (overrelaxation sub-step; 32 of the 40 update launches per sweep)",
+                "achieved": ach, "peak": peak[0], "unit": "GB/s", "frac": ach / peak[0], "peak_source": peak[1],
+                "frac_of_8TBs": ach / 8000.0, "algorithmic_bytes_per_launch": bpu * (V // 2),
+                "bytes_per_link_update": bpu, "avg_launch_ms": or_ms, "hb_avg_launch_ms": hb_ms,
+                "hb_achieved": (bpu * (V // 2) / (hb_ms * 1e-3) / 1e9) if hb_ms else None,
+                "update_kernels_share_of_step": (tim["or_ms"] + tim["hb_ms"]) / res["ms"],
+                "traffic": ncu_traffic(f"su{Nc}_{precision}_{'recon12' if recon12 else 'full'}_or")}
+    return {"value": value, "ms_per_step": res["ms"] / steps, "gflops": n_ranks * flops_step / t_step / 1e9,
+            "effective_gbs": n_ranks * bpu * updates_step / t_step / 1e9, "roofline": roof}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="su3_48", choices=sorted(WORKLOADS))
+    ap.add_argument("--precision", default="fp64", choices=["fp32", "fp64"])
+    ap.add_argument("--storage", default="full", choices=["full", "recon12"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "specialised", "generic"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-variants", action="store_true", help="skip the extra fp32 / 12-real runs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    wl = WORKLOADS[args.workload]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, wl, rank)
+
+    import torch
+    import paper_1112_4533_b200 as su          # raises if libsugauge.so is missing: no fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    warmup = max(args.warmup, 3)
+    peak = measured_peaks()
+    recon12 = args.storage == "recon12"
+
+    def timed(precision, r12, kernel, steps, wu, clocks):
+        lat = make_lattice(su, wl, precision, r12, kernel, rank, local)
+        res = time_resident(torch, dist, lat, wl, steps, wu, clocks, local)
+        if dist is not None:                   # max over ranks of the device time
+            t = torch.tensor([res["ms"]], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            res["ms"] = float(t.item())
+        return lat, res
+
+    lat, res = timed(args.precision, recon12, args.kernel, args.steps, warmup, True)
+    main_num = variant_numbers(wl, args.precision, recon12, res, args.steps, world, peak)
+    e2e = None
+    if not args.no_e2e:
+        r = time_e2e(torch, dist, lat, wl, max(1, args.e2e_steps))
+        if dist is not None:
+            t = torch.tensor([r["ms"]], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            r["ms"] = float(t.item())
+        e2e = {"value": world * (N_HB + N_OR) * 4 * wl["L"] ** 4 / (r["ms"] / r["steps"] * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"], "ms_per_step": r["ms"] / r["steps"],
+               "steps": r["steps"], "what": "su_import_links(pinned host, canonical doubles) + step + su_export_links"}
+    lat.close()
+    del lat
+
+    variants = []
+    if not args.no_variants and wl["Nc"] <= 4:
+        combos = [(p, s) for p in ("fp64", "fp32") for s in ((False, True) if wl["Nc"] == 3 else (False,))]
+        for p, r12 in combos:
+            if (p, r12) == (args.precision, recon12):
+                continue
+            k = max(3, min(args.steps, 10))
+            l2, r2 = timed(p, r12, args.kernel, k, 3, False)
+            n = variant_numbers(wl, p, r12, r2, k, world, peak)
+            variants.append({"precision": p, "storage": "recon12" if r12 else "full", "steps": k, "value": n["value"],
+                             "ms_per_step": n["ms_per_step"], "gflops": n["gflops"],
+                             "roofline_frac": n["roofline"]["frac"] if n["roofline"] else None,
+                             "or_launch_ms": n["roofline"]["avg_launch_ms"] if n["roofline"] else None,
+                             "hb_launch_ms": n["roofline"]["hb_avg_launch_ms"] if n["roofline"] else None})
+            l2.close()
+            del l2
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(wl, args.precision, recon12)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": main_num["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": warmup, "ms_per_step": main_num["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32", "data": "synthetic",
+                "config": {"workload": args.workload, "Nc": wl["Nc"], "lattice": f"{wl['L']}^4", "beta": wl["beta"],
+                           "start": f"{wl['start']} (Philox seed {wl['seed']} + rank)", "sweep": "1 heatbath + 4 overrelaxation",
+                           "step": "su_sweep(1,4) + su_reunitarize + su_plaquette + su_polyakov" if wl["Nc"] > 2
+                                   else "su_sweep(1,4) + su_plaquette + su_polyakov",
+                           "storage": args.storage, "kernel": args.kernel,
+                           "lattice_bytes": su.lattice_bytes(wl["Nc"], (wl["L"],) * 4, args.precision, recon12),
+                           "l2": "inputs larger than L2 (no flush)" if su.lattice_bytes(wl["Nc"], (wl["L"],) * 4, args.precision, recon12) > 3 * 126e6
+                                 else "lattice fits in L2: L2-resident by design, HBM fraction not meaningful",
+                           "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)"},
+                "gflops": main_num["gflops"], "effective_hbm_gbs": main_num["effective_gbs"],
+                "flop_formula": "13*mm+10Nc^2 + n_sub*(23+56Nc) [OR] / n_sub*(57+13*1.05+56Nc) [HB], mm=8Nc^3-2Nc^2 (DESIGN.md)",
+                "roofline": main_num["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": res["launches"],
+                "clocks": res["clocks"], "plaquette": res["plaquette"], "polyakov": res["polyakov"],
+                "kp_exhausted": res["kp_exhausted"], "variants": variants}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
