@@ -38,11 +38,11 @@ __global__ void __launch_bounds__(REDUCE_BLOCK) k_plaquette(const AuxArgs a) {
         for (int mu = 0; mu < 3; ++mu)
 #pragma unroll 1
             for (int nu = mu + 1; nu < 4; ++nu) {
-                IO::template load<true>(IO::plane((const void*)a.links, a.g, mu, p), Vh, cb, A);
-                IO::template load<true>(IO::plane((const void*)a.links, a.g, nu, 1 - p), Vh, fwd[mu], B);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, p), Vh, cb, A);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, 1 - p), Vh, fwd[mu], B);
                 M::mul_nn(A, B, P);
-                IO::template load<true>(IO::plane((const void*)a.links, a.g, nu, p), Vh, cb, A);
-                IO::template load<true>(IO::plane((const void*)a.links, a.g, mu, 1 - p), Vh, fwd[nu], B);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, p), Vh, cb, A);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, 1 - p), Vh, fwd[nu], B);
                 M::mul_nn(A, B, Q);
                 acc += (double)M::retr_nd(P, Q);
             }
@@ -65,10 +65,10 @@ __global__ void __launch_bounds__(REDUCE_BLOCK) k_polyakov(const AuxArgs a) {
         const int y = (int)((xs / (unsigned)a.g.L[0]) % (unsigned)a.g.L[1]);
         const int z = (int)(xs / ((unsigned)a.g.L[0] * a.g.L[1]));
         C P[NC * NC], A[NC * NC], Q[NC * NC];
-        IO::template load<true>(IO::plane((const void*)a.links, a.g, 3, (x + y + z) & 1), a.g.Vh, cb_of(a.g, x, y, z, 0), P);
+        IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z) & 1), a.g.Vh, cb_of(a.g, x, y, z, 0), P);
 #pragma unroll 1
         for (int t = 1; t < a.g.L[3]; ++t) {
-            IO::template load<true>(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), a.g.Vh, cb_of(a.g, x, y, z, t), A);
+            IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), a.g.Vh, cb_of(a.g, x, y, z, t), A);
             M::mul_nn(P, A, Q);
 #pragma unroll(UNR ? NC * NC : 1)
             for (int e = 0; e < NC * NC; ++e) P[e] = Q[e];
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
     if (!link_of_thread(a.g, blockIdx.x * 128u + threadIdx.x, mu, p, cb)) return;
     typename IO::T2* pl = IO::plane(a.links, a.g, mu, p);
     cx<T> U[NC * NC];
-    IO::template load<false>(pl, a.g.Vh, cb, U);
+    IO::template load<LD_PLAIN>(pl, a.g.Vh, cb, U);
     if (NC == 2) {
         T n = Fn<T>::sqrt((U[0].re * U[0].re + U[0].im * U[0].im) + (U[1].re * U[1].re + U[1].im * U[1].im));
         U[0] = mk<T>(U[0].re / n, U[0].im / n);
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(128) k_export(const AuxArgs a) {
     const int t = (int)(r / (unsigned)a.g.L[2]);
     const int p = (x + y + z + t) & 1;
     cx<T> U[NC * NC];
-    IO::template load<false>(IO::plane((const void*)a.links, a.g, mu, p), a.g.Vh, s >> 1, U);
+    IO::template load<LD_PLAIN>(IO::plane((const void*)a.links, a.g, mu, p), a.g.Vh, s >> 1, U);
     double2* dst = (double2*)a.staging + (size_t)l * NC * NC;
     for (int e = 0; e < NC * NC; ++e) dst[e] = make_double2((double)U[e].re, (double)U[e].im);
 }

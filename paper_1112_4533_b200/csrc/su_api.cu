@@ -83,6 +83,18 @@ bool dims_ok(int Nc, int Lx, int Ly, int Lz, int Lt) {
 
 int elems_per_link(int Nc, su_storage s) { return Nc == 2 ? 2 : (s == SU_STORE_RECON12 ? 6 : Nc * Nc); }
 
+// Traversal order of the update kernel: the largest divisor Zc of Lz for
+// which one (Zc z-planes) x (one time slice) x (all 8 link planes) chunk stays under 16 MB, so that the
+// three chunks in flight (t-1, t, t+1) sit in L2 together. Measured at 48^4: DRAM traffic 1.34x -> 1.08x
+// of the algorithmic bytes (profiles/r01a, r01b).
+int traversal_z_chunk(const Geom& g, size_t link_bytes) {
+    const size_t plane = (size_t)g.L[0] * g.L[1] * 4 * link_bytes;   // one z-plane of one time slice, 4 directions
+    int zc = 1;
+    for (int d = 1; d <= g.L[2]; ++d)
+        if (g.L[2] % d == 0 && plane * (size_t)d <= ((size_t)16 << 20)) zc = d;
+    return zc;
+}
+
 #define SU_BY_NC(h, FN, ...)                                                   \
     ([&]() -> cudaError_t {                                                    \
         switch ((h)->Nc) {                                                     \
@@ -218,9 +230,10 @@ su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precis
     h->g.Lxh = Lx / 2;
     h->V = (size_t)Lx * Ly * Lz * Lt;
     h->g.Vh = (unsigned)(h->V / 2);
+    h->var.store = Nc == 2 ? STORE_QUAT : (o.storage == SU_STORE_RECON12 ? STORE_RECON12 : STORE_FULL);
+    h->g.Zc = traversal_z_chunk(h->g, (size_t)elems_per_link(Nc, o.storage) * 2 * (p == SU_FP64 ? 8 : 4));
     h->prec = p;
     h->var.Nc = Nc; h->var.prec = (int)p;
-    h->var.store = Nc == 2 ? STORE_QUAT : (o.storage == SU_STORE_RECON12 ? STORE_RECON12 : STORE_FULL);
     h->var.generic = (o.kernel == SU_KERNEL_GENERIC) || (o.kernel == SU_KERNEL_AUTO && Nc > 4);
     h->stream = (cudaStream_t)o.stream;
 

@@ -43,6 +43,7 @@ struct Geom {
     int L[4];
     int Lxh;        // Lx / 2
     unsigned Vh;    // V / 2 = sites per parity
+    int Zc;         // z-chunk of the update kernel's traversal order (divides Lz)
 };
 
 __device__ __forceinline__ void decode_cb(const Geom& g, unsigned cb, int parity, int c[4]) {
@@ -79,6 +80,17 @@ template <class T> __device__ __forceinline__ void su3_third_row(cx<T>* m) {   /
     m[8] = conj(m[0] * m[4] - m[1] * m[3]);
 }
 
+// Load / store flavours: LD_PLAIN = ld.global (read-write data), LD_RO = ld.global.nc (neighbour links,
+// read-only during a sub-step, kept in L1/L2 for re-use), LD_STREAM = ld.global.cs / st.global.cs (the
+// link being updated: touched once per sub-step, so it should not displace re-used lines).
+enum : int { LD_PLAIN = 0, LD_RO = 1, LD_STREAM = 2 };
+template <class T, int LD> __device__ __forceinline__ typename V2<T>::type ldg2(const typename V2<T>::type* p) {
+    return LD == LD_RO ? __ldg(p) : (LD == LD_STREAM ? __ldcs(p) : *p);
+}
+template <class T, bool STREAM> __device__ __forceinline__ void stg2(typename V2<T>::type* p, typename V2<T>::type v) {
+    if (STREAM) __stcs(p, v); else *p = v;
+}
+
 template <int NC, class T, int STORE, bool UNR> struct LinkIO {
     typedef typename V2<T>::type T2;
     static constexpr int E = LinkElems<NC, STORE>::E;
@@ -91,30 +103,31 @@ template <int NC, class T, int STORE, bool UNR> struct LinkIO {
     static __device__ __forceinline__ T2* plane(void* base, const Geom& g, int mu, int par) {
         return (T2*)base + (size_t)(mu * 2 + par) * E * g.Vh;
     }
-    template <bool RO>
+    template <int LD>
     static __device__ __forceinline__ void load(const T2* __restrict__ pl, unsigned Vh, unsigned cb, cx<T>* m) {
         if (STORE == STORE_QUAT) {
-            T2 v0 = RO ? __ldg(pl + cb) : pl[cb];
-            T2 v1 = RO ? __ldg(pl + Vh + cb) : pl[Vh + cb];
+            T2 v0 = ldg2<T, LD>(pl + cb);
+            T2 v1 = ldg2<T, LD>(pl + Vh + cb);
             // eq 6: [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]], v0 = (a0,a1), v1 = (a2,a3)
             m[0] = mk<T>(v0.x, v1.y);  m[1] = mk<T>(v1.x, v0.y);
             m[2] = mk<T>(-v1.x, v0.y); m[3] = mk<T>(v0.x, -v1.y);
         } else {
 #pragma unroll(UNR ? E : 1)
             for (int e = 0; e < E; ++e) {
-                T2 v = RO ? __ldg(pl + (size_t)e * Vh + cb) : pl[(size_t)e * Vh + cb];
+                T2 v = ldg2<T, LD>(pl + (size_t)e * Vh + cb);
                 m[e] = mk<T>(v.x, v.y);
             }
             if (STORE == STORE_RECON12) su3_third_row(m);
         }
     }
+    template <bool STREAM = false>
     static __device__ __forceinline__ void store(T2* __restrict__ pl, unsigned Vh, unsigned cb, const cx<T>* m) {
         if (STORE == STORE_QUAT) {
-            pl[cb]      = V2<T>::make(m[0].re, m[1].im);
-            pl[Vh + cb] = V2<T>::make(m[1].re, m[0].im);
+            stg2<T, STREAM>(pl + cb,      V2<T>::make(m[0].re, m[1].im));
+            stg2<T, STREAM>(pl + Vh + cb, V2<T>::make(m[1].re, m[0].im));
         } else {
 #pragma unroll(UNR ? E : 1)
-            for (int e = 0; e < E; ++e) pl[(size_t)e * Vh + cb] = V2<T>::make(m[e].re, m[e].im);
+            for (int e = 0; e < E; ++e) stg2<T, STREAM>(pl + (size_t)e * Vh + cb, V2<T>::make(m[e].re, m[e].im));
         }
     }
 };

@@ -5,19 +5,9 @@
 
 #include "../../include/su_gauge.h"
 #include "su_device.cuh"
+#include "update_kernel.cuh"
 
 namespace sug {
-
-struct UpdateArgs {
-    void* links;
-    Geom g;
-    int parity, mu;
-    double beta;
-    uint32_t k0, k1, sweep, pass;
-    const uint32_t* sweep_ptr;         // device; when non-NULL the sweep counter is read from here (graph replay)
-    uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
-    unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
-};
 
 struct Variant {
     int Nc;

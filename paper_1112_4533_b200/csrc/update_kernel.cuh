@@ -1,0 +1,216 @@
+// update_kernel.cuh — the staple + link-update kernel (heatbath / overrelaxation) for one
+// (parity, mu) sub-step of the sweep ("eight steps" per pass).
+//
+// One thread owns one link U_mu(x), x of the given parity. It gathers the 18 staple
+// links (eq 9) from the SoA planes with coalesced 64/128-bit loads, forms
+// W = U S^dagger (step 2), runs the SU(2) subgroup loop (steps 3-5) and stores the link.
+//   UNR = true : matrices fully unrolled into registers (specialised SU(3)/SU(4))
+//   UNR = false: rolled loops over local arrays (generic SU(Nc))
+//
+// Thread -> site mapping: the thread index walks the lattice as
+// (z-chunk, t, z within chunk, y, x/2), so that the data first touched at t+1 is touched again
+// (at t and t-1) before 2 * Zc/Lz time slices of all planes have streamed through L2.
+#pragma once
+#include "su_device.cuh"
+
+namespace sug {
+
+struct UpdateArgs {
+    void* links;
+    Geom g;
+    int parity, mu;
+    double beta;
+    uint32_t k0, k1, sweep, pass;
+    const uint32_t* sweep_ptr;         // device; when non-NULL the sweep counter is read from here (graph replay)
+    uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
+    unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
+};
+
+// The site a thread works on and the checkerboard-index offsets of its 8 neighbours.
+struct SiteNbr {
+    unsigned cb;        // checkerboard index of x
+    uint32_t lex;       // lexicographic site index of x (RNG counter word c0)
+    int dp[4], dm[4];   // cb(x + e_d) - cb(x), cb(x - e_d) - cb(x)   (periodic)
+};
+
+__device__ __forceinline__ int sel4(int i, int v0, int v1, int v2, int v3) {
+    return i == 0 ? v0 : (i == 1 ? v1 : (i == 2 ? v2 : v3));
+}
+
+// traversal index -> site; all indices stay in registers (no dynamically indexed arrays)
+__device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int parity, SiteNbr& s) {
+    const unsigned row = (unsigned)g.Lxh, pl = row * (unsigned)g.L[1];
+    const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.L[3];
+    const unsigned zc = tix / span;  unsigned r = tix - zc * span;
+    const unsigned t = r / grp;      r -= t * grp;
+    const unsigned zi = r / pl;      r -= zi * pl;
+    const unsigned y = r / row;
+    const unsigned xh = r - y * row;
+    const unsigned z = zc * (unsigned)g.Zc + zi;
+    const int sy = (int)row, sz = (int)pl, st = (int)(pl * (unsigned)g.L[2]);
+    const int q = (int)((y + z + t + (unsigned)parity) & 1u);          // x = 2 xh + q
+    s.cb = xh + row * (y + (unsigned)g.L[1] * (z + (unsigned)g.L[2] * t));
+    s.lex = 2u * s.cb + (unsigned)q;
+    s.dp[0] = q ? ((int)xh + 1 == g.Lxh ? 1 - g.Lxh : 1) : 0;
+    s.dm[0] = q ? 0 : (xh == 0 ? g.Lxh - 1 : -1);
+    s.dp[1] = ((int)y + 1 == g.L[1]) ? -(g.L[1] - 1) * sy : sy;
+    s.dm[1] = (y == 0) ? (g.L[1] - 1) * sy : -sy;
+    s.dp[2] = ((int)z + 1 == g.L[2]) ? -(g.L[2] - 1) * sz : sz;
+    s.dm[2] = (z == 0) ? (g.L[2] - 1) * sz : -sz;
+    s.dp[3] = ((int)t + 1 == g.L[3]) ? -(g.L[3] - 1) * st : st;
+    s.dm[3] = (t == 0) ? (g.L[3] - 1) * st : -st;
+}
+
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
+    typedef LinkIO<NC, T, STORE, UNR> IO;
+    typedef Mat<NC, T, UNR> M;
+    typedef cx<T> C;
+    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tix < a.g.Vh;
+    unsigned att_total = 0, exhausted = 0;
+    if (active) {
+        const int p = a.parity, mu = a.mu;
+        const unsigned Vh = a.g.Vh;
+        SiteNbr s;
+        site_of_thread(a.g, tix, p, s);
+        const unsigned cb = s.cb;
+        const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+
+        C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
+        M::zero(S);
+        const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {
+            const int nu = k + (k >= mu ? 1 : 0);
+            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+            const typename IO::T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
+            const typename IO::T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
+            // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+            IO::template load<LD_RO>(pl_nu_s, Vh, cb, A);
+            IO::template load<LD_RO>(pl_mu_o, Vh, cb + (unsigned)dpnu, B);
+            M::mul_nn(A, B, P);
+            IO::template load<LD_RO>(pl_nu_o, Vh, cb + (unsigned)dpmu, A);
+            M::acc_nd(S, P, A);
+            // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
+            IO::template load<LD_RO>(pl_nu_o, Vh, cb + (unsigned)dmnu, A);
+            IO::template load<LD_RO>(pl_mu_o, Vh, cb + (unsigned)dmnu, B);
+            M::mul_dn(A, B, P);
+            IO::template load<LD_RO>(pl_nu_s, Vh, cb + (unsigned)(dmnu + dpmu), A);
+            M::acc_nn(S, P, A);
+        }
+        typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
+        C* U = A;
+        C* W = B;
+        IO::template load<LD_STREAM>(pl_self, Vh, cb, U);
+        M::mul_nd(U, S, W);                                   // W = U S^dagger
+        update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex,
+                                           a.sweep_ptr ? *a.sweep_ptr : a.sweep,
+                                           pack_c2(0, (int)a.pass, p, mu, 0),
+                                           a.attempts ? a.attempts + cb : nullptr, (size_t)Vh,
+                                           att_total, exhausted);
+        IO::template store<true>(pl_self, Vh, cb, U);
+    }
+    if (KIND == KIND_HB) {
+        for (int o = 16; o > 0; o >>= 1) {
+            att_total += __shfl_down_sync(0xffffffffu, att_total, o);
+            exhausted += __shfl_down_sync(0xffffffffu, exhausted, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            if (att_total) atomicAdd(a.counters, (unsigned long long)att_total);
+            if (exhausted) atomicAdd(a.counters + 1, (unsigned long long)exhausted);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// SU(2) in the 4-real parameterisation U = a0 + i a.sigma (eqs 6-8): links,
+// staple and update are quaternion arithmetic. Same algebra as the matrix path:
+// W = U S^bar, k = |W|, u~ = W/k, a = v u~^bar (heatbath, eq 14) or (u~^bar)^2 (eq 17), U' = a U.
+// ------------------------------------------------------------------------------------------
+template <class T, int LD> __device__ __forceinline__ void qload(const typename V2<T>::type* __restrict__ pl, unsigned Vh, unsigned cb, T q[4]) {
+    typename V2<T>::type v0 = ldg2<T, LD>(pl + cb);
+    typename V2<T>::type v1 = ldg2<T, LD>(pl + Vh + cb);
+    q[0] = v0.x; q[1] = v0.y; q[2] = v1.x; q[3] = v1.y;
+}
+template <class T> __device__ __forceinline__ void qconj(const T a[4], T o[4]) { o[0] = a[0]; o[1] = -a[1]; o[2] = -a[2]; o[3] = -a[3]; }
+
+template <class T, int KIND, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) {
+    typedef typename V2<T>::type T2;
+    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tix < a.g.Vh;
+    unsigned att_total = 0, exhausted = 0;
+    if (active) {
+        const int p = a.parity, mu = a.mu;
+        const unsigned Vh = a.g.Vh;
+        SiteNbr s;
+        site_of_thread(a.g, tix, p, s);
+        const unsigned cb = s.cb;
+        const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+        const T2* base = (const T2*)a.links;
+        auto plane = [&](int d, int par) { return base + (size_t)(d * 2 + par) * 2 * Vh; };
+        T S[4] = {0, 0, 0, 0}, A[4], B[4], Cq[4], P[4], Q[4];
+        const T2* pl_mu_o = plane(mu, 1 - p);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int nu = k + (k >= mu ? 1 : 0);
+            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+            const T2* pl_nu_s = plane(nu, p);
+            const T2* pl_nu_o = plane(nu, 1 - p);
+            qload<T, LD_RO>(pl_nu_s, Vh, cb, A);
+            qload<T, LD_RO>(pl_mu_o, Vh, cb + (unsigned)dpnu, B);
+            qload<T, LD_RO>(pl_nu_o, Vh, cb + (unsigned)dpmu, Cq);
+            quat_mul(A, B, P); qconj(Cq, A); quat_mul(P, A, Q);
+            S[0] += Q[0]; S[1] += Q[1]; S[2] += Q[2]; S[3] += Q[3];
+            qload<T, LD_RO>(pl_nu_o, Vh, cb + (unsigned)dmnu, A);
+            qload<T, LD_RO>(pl_mu_o, Vh, cb + (unsigned)dmnu, B);
+            qload<T, LD_RO>(pl_nu_s, Vh, cb + (unsigned)(dmnu + dpmu), Cq);
+            qconj(A, P); quat_mul(P, B, Q); quat_mul(Q, Cq, P);
+            S[0] += P[0]; S[1] += P[1]; S[2] += P[2]; S[3] += P[3];
+        }
+        T2* pl_self = (T2*)a.links + (size_t)(mu * 2 + p) * 2 * Vh;
+        T U[4], W[4], a4[4] = {1, 0, 0, 0};
+        qload<T, LD_STREAM>(pl_self, Vh, cb, U);
+        qconj(S, A);
+        quat_mul(U, A, W);
+        T k = Fn<T>::sqrt(W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+        bool ok = (k > (T)0) && Fn<T>::finite(k);
+        int used = 0;
+        if (ok) {
+            T ud[4] = {W[0] / k, -W[1] / k, -W[2] / k, -W[3] / k};
+            if (KIND == KIND_HB) {
+                T v[4];
+                used = kp_draw<T>((T)a.beta * k, a.k0, a.k1, s.lex, a.sweep_ptr ? *a.sweep_ptr : a.sweep,
+                                  pack_c2(0, (int)a.pass, p, mu, 0), v);
+                if (used) quat_mul(v, ud, a4); else ok = false;
+            } else {
+                quat_mul(ud, ud, a4);
+            }
+        }
+        if (KIND == KIND_HB) {
+            att_total = (unsigned)used;
+            exhausted = ok ? 0u : 1u;
+            if (a.attempts) a.attempts[cb] = (uint8_t)(used > 255 ? 255 : used);
+        }
+        if (ok) {
+            quat_mul(a4, U, P);
+            stg2<T, true>(pl_self + cb, V2<T>::make(P[0], P[1]));
+            stg2<T, true>(pl_self + Vh + cb, V2<T>::make(P[2], P[3]));
+        }
+    }
+    if (KIND == KIND_HB) {
+        for (int o = 16; o > 0; o >>= 1) {
+            att_total += __shfl_down_sync(0xffffffffu, att_total, o);
+            exhausted += __shfl_down_sync(0xffffffffu, exhausted, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            if (att_total) atomicAdd(a.counters, (unsigned long long)att_total);
+            if (exhausted) atomicAdd(a.counters + 1, (unsigned long long)exhausted);
+        }
+    }
+}
+
+}  // namespace sug
