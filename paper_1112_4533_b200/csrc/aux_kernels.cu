@@ -1,6 +1,6 @@
 // aux_kernels.cu — everything on the path except the link update: plaquette and Polyakov-loop
 // reductions (fp64 accumulation, warp shuffle + block + final pass), reunitarisation, cold / hot
-// start, and the SoA <-> canonical-layout conversion used by export / import.
+// start, and the tiled-SoA <-> canonical-layout conversion used by export / import.
 // Compiled once per colour count with -DSUG_NC=<Nc>.
 #include "su_internal.h"
 
@@ -38,11 +38,11 @@ __global__ void __launch_bounds__(REDUCE_BLOCK) k_plaquette(const AuxArgs a) {
         for (int mu = 0; mu < 3; ++mu)
 #pragma unroll 1
             for (int nu = mu + 1; nu < 4; ++nu) {
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, p), Vh, cb, A);
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, 1 - p), Vh, fwd[mu], B);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, p), cb, A);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, 1 - p), fwd[mu], B);
                 M::mul_nn(A, B, P);
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, p), Vh, cb, A);
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, 1 - p), Vh, fwd[nu], B);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, p), cb, A);
+                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, 1 - p), fwd[nu], B);
                 M::mul_nn(A, B, Q);
                 acc += (double)M::retr_nd(P, Q);
             }
@@ -65,10 +65,10 @@ __global__ void __launch_bounds__(REDUCE_BLOCK) k_polyakov(const AuxArgs a) {
         const int y = (int)((xs / (unsigned)a.g.L[0]) % (unsigned)a.g.L[1]);
         const int z = (int)(xs / ((unsigned)a.g.L[0] * a.g.L[1]));
         C P[NC * NC], A[NC * NC], Q[NC * NC];
-        IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z) & 1), a.g.Vh, cb_of(a.g, x, y, z, 0), P);
+        IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z) & 1), cb_of(a.g, x, y, z, 0), P);
 #pragma unroll 1
         for (int t = 1; t < a.g.L[3]; ++t) {
-            IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), a.g.Vh, cb_of(a.g, x, y, z, t), A);
+            IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), cb_of(a.g, x, y, z, t), A);
             M::mul_nn(P, A, Q);
 #pragma unroll(UNR ? NC * NC : 1)
             for (int e = 0; e < NC * NC; ++e) P[e] = Q[e];
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
     if (!link_of_thread(a.g, blockIdx.x * 128u + threadIdx.x, mu, p, cb)) return;
     typename IO::T2* pl = IO::plane(a.links, a.g, mu, p);
     cx<T> U[NC * NC];
-    IO::template load<LD_PLAIN>(pl, a.g.Vh, cb, U);
+    IO::template load<LD_PLAIN>(pl, cb, U);
     if (NC == 2) {
         T n = Fn<T>::sqrt((U[0].re * U[0].re + U[0].im * U[0].im) + (U[1].re * U[1].re + U[1].im * U[1].im));
         U[0] = mk<T>(U[0].re / n, U[0].im / n);
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
         gram_schmidt_rows<NC, T>(U, NC);
         fix_determinant_phase<NC, T>(U);
     }
-    IO::store(pl, a.g.Vh, cb, U);
+    IO::store(pl, cb, U);
 }
 
 template <int NC, class T, int STORE, bool UNR>
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(128) k_init_cold(const AuxArgs a) {
     cx<T> U[NC * NC];
     for (int i = 0; i < NC; ++i)
         for (int j = 0; j < NC; ++j) U[i * NC + j] = mk<T>(i == j ? (T)1 : (T)0, (T)0);
-    IO::store(IO::plane(a.links, a.g, mu, p), a.g.Vh, cb, U);
+    IO::store(IO::plane(a.links, a.g, mu, p), cb, U);
 }
 
 // Hot start (readings R12, R20): Haar SU(Nc) per link from Philox blocks
@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(128) k_init_hot(const AuxArgs a) {
     }
     cx<T> U[NC * NC];
     for (int e = 0; e < NC * NC; ++e) U[e] = mk<T>((T)Md[e].re, (T)Md[e].im);
-    IO::store(IO::plane(a.links, a.g, mu, p), a.g.Vh, cb, U);
+    IO::store(IO::plane(a.links, a.g, mu, p), cb, U);
 }
 
 // SoA -> canonical [site][mu][row][col][re,im] doubles for lexicographic sites [site0, site0+nsites)
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(128) k_export(const AuxArgs a) {
     const int t = (int)(r / (unsigned)a.g.L[2]);
     const int p = (x + y + z + t) & 1;
     cx<T> U[NC * NC];
-    IO::template load<LD_PLAIN>(IO::plane((const void*)a.links, a.g, mu, p), a.g.Vh, s >> 1, U);
+    IO::template load<LD_PLAIN>(IO::plane((const void*)a.links, a.g, mu, p), s >> 1, U);
     double2* dst = (double2*)a.staging + (size_t)l * NC * NC;
     for (int e = 0; e < NC * NC; ++e) dst[e] = make_double2((double)U[e].re, (double)U[e].im);
 }
@@ -275,7 +275,7 @@ __global__ void __launch_bounds__(128) k_import(const AuxArgs a) {
     const double2* src = (const double2*)a.staging + (size_t)l * NC * NC;
     cx<T> U[NC * NC];
     for (int e = 0; e < NC * NC; ++e) { double2 v = src[e]; U[e] = mk<T>((T)v.x, (T)v.y); }
-    IO::store(IO::plane(a.links, a.g, mu, p), a.g.Vh, s >> 1, U);
+    IO::store(IO::plane(a.links, a.g, mu, p), s >> 1, U);
 }
 
 // ---- dispatch -----------------------------------------------------------------------------

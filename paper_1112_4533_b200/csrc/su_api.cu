@@ -82,6 +82,8 @@ bool dims_ok(int Nc, int Lx, int Ly, int Lz, int Lt) {
 }
 
 int elems_per_link(int Nc, su_storage s) { return Nc == 2 ? 2 : (s == SU_STORE_RECON12 ? 6 : Nc * Nc); }
+// sites stored per (mu, parity) plane: V/2 rounded up to whole tiles of LINK_TILE sites
+size_t plane_sites(size_t Vh) { return (Vh + LINK_TILE - 1) / LINK_TILE * LINK_TILE; }
 
 // Traversal order of the update kernel: the largest divisor Zc of Lz for
 // which one (Zc z-planes) x (one time slice) x (all 8 link planes) chunk stays under 16 MB, so that the
@@ -200,8 +202,8 @@ size_t su_lattice_bytes(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, 
     if (!dims_ok(Nc, Lx, Ly, Lz, Lt) || (p != SU_FP32 && p != SU_FP64)) return 0;
     if (s != SU_STORE_FULL && s != SU_STORE_RECON12) return 0;
     if (s == SU_STORE_RECON12 && Nc != 3) return 0;
-    const size_t V = (size_t)Lx * Ly * Lz * Lt;
-    const size_t b = 4 * V * (size_t)elems_per_link(Nc, s) * 2 * (p == SU_FP64 ? 8 : 4);
+    const size_t Vhp = plane_sites((size_t)Lx * Ly * Lz * Lt / 2);
+    const size_t b = 8 * Vhp * (size_t)elems_per_link(Nc, s) * 2 * (p == SU_FP64 ? 8 : 4);
     return (b + 255) / 256 * 256;
 }
 
@@ -230,6 +232,7 @@ su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precis
     h->g.Lxh = Lx / 2;
     h->V = (size_t)Lx * Ly * Lz * Lt;
     h->g.Vh = (unsigned)(h->V / 2);
+    h->g.Vhp = (unsigned)plane_sites(h->V / 2);
     h->var.store = Nc == 2 ? STORE_QUAT : (o.storage == SU_STORE_RECON12 ? STORE_RECON12 : STORE_FULL);
     h->g.Zc = traversal_z_chunk(h->g, (size_t)elems_per_link(Nc, o.storage) * 2 * (p == SU_FP64 ? 8 : 4));
     h->prec = p;

@@ -39,10 +39,13 @@ template <class T> __device__ __forceinline__ void mad_ca(cx<T>& acc, cx<T> a, c
 // ------------------------------------------------------------------------------------------
 // Geometry (readings R7): even extents, periodic, checkerboard index cb = i/2.
 // ------------------------------------------------------------------------------------------
+constexpr int LINK_TILE = 32;   // sites per AoSoA tile of the link storage (one warp-wide row per matrix element)
+
 struct Geom {
     int L[4];
     int Lxh;        // Lx / 2
     unsigned Vh;    // V / 2 = sites per parity
+    unsigned Vhp;   // Vh rounded up to a multiple of LINK_TILE = sites per stored plane
     int Zc;         // z-chunk of the update kernel's traversal order (divides Lz)
 };
 
@@ -68,7 +71,12 @@ __device__ __forceinline__ unsigned cb_shift(const Geom& g, const int c[4], int 
 }
 
 // ------------------------------------------------------------------------------------------
-// Link I/O on the SoA layout links[mu][parity][elem][cb] of (re,im) pairs.
+// Link I/O on the tiled structure-of-arrays layout
+//     links[mu][parity][cb / 32][elem][cb % 32]   of (re,im) pairs:
+// a warp reading one matrix element of 32 consecutive sites issues one coalesced 256 B (fp32) /
+// 512 B (fp64) request, the E elements of a link sit at compile-time offsets e * 32 from one base
+// address (one address computation per link instead of one per element), and the E rows of a
+// tile are one contiguous E * 512 B piece of DRAM.
 // ------------------------------------------------------------------------------------------
 template <int NC, int STORE> struct LinkElems {
     static constexpr int E = (STORE == STORE_QUAT) ? 2 : ((STORE == STORE_RECON12) ? 6 : NC * NC);
@@ -98,36 +106,45 @@ template <int NC, class T, int STORE, bool UNR> struct LinkIO {
     static_assert(STORE != STORE_RECON12 || NC == 3, "two-row storage is SU(3) only");
 
     static __device__ __forceinline__ const T2* plane(const void* base, const Geom& g, int mu, int par) {
-        return (const T2*)base + (size_t)(mu * 2 + par) * E * g.Vh;
+        return (const T2*)base + (size_t)(mu * 2 + par) * E * g.Vhp;
     }
     static __device__ __forceinline__ T2* plane(void* base, const Geom& g, int mu, int par) {
-        return (T2*)base + (size_t)(mu * 2 + par) * E * g.Vh;
+        return (T2*)base + (size_t)(mu * 2 + par) * E * g.Vhp;
+    }
+    // address of element 0 of site cb in a plane; element e is at + e * LINK_TILE
+    static __device__ __forceinline__ const T2* site(const T2* pl, unsigned cb) {
+        return pl + (size_t)(cb / LINK_TILE) * (E * LINK_TILE) + (cb % LINK_TILE);
+    }
+    static __device__ __forceinline__ T2* site(T2* pl, unsigned cb) {
+        return pl + (size_t)(cb / LINK_TILE) * (E * LINK_TILE) + (cb % LINK_TILE);
     }
     template <int LD>
-    static __device__ __forceinline__ void load(const T2* __restrict__ pl, unsigned Vh, unsigned cb, cx<T>* m) {
+    static __device__ __forceinline__ void load(const T2* __restrict__ pl, unsigned cb, cx<T>* m) {
+        pl = site(pl, cb);
         if (STORE == STORE_QUAT) {
-            T2 v0 = ldg2<T, LD>(pl + cb);
-            T2 v1 = ldg2<T, LD>(pl + Vh + cb);
+            T2 v0 = ldg2<T, LD>(pl);
+            T2 v1 = ldg2<T, LD>(pl + LINK_TILE);
             // eq 6: [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]], v0 = (a0,a1), v1 = (a2,a3)
             m[0] = mk<T>(v0.x, v1.y);  m[1] = mk<T>(v1.x, v0.y);
             m[2] = mk<T>(-v1.x, v0.y); m[3] = mk<T>(v0.x, -v1.y);
         } else {
 #pragma unroll(UNR ? E : 1)
             for (int e = 0; e < E; ++e) {
-                T2 v = ldg2<T, LD>(pl + (size_t)e * Vh + cb);
+                T2 v = ldg2<T, LD>(pl + e * LINK_TILE);
                 m[e] = mk<T>(v.x, v.y);
             }
             if (STORE == STORE_RECON12) su3_third_row(m);
         }
     }
     template <bool STREAM = false>
-    static __device__ __forceinline__ void store(T2* __restrict__ pl, unsigned Vh, unsigned cb, const cx<T>* m) {
+    static __device__ __forceinline__ void store(T2* __restrict__ pl, unsigned cb, const cx<T>* m) {
+        pl = site(pl, cb);
         if (STORE == STORE_QUAT) {
-            stg2<T, STREAM>(pl + cb,      V2<T>::make(m[0].re, m[1].im));
-            stg2<T, STREAM>(pl + Vh + cb, V2<T>::make(m[1].re, m[0].im));
+            stg2<T, STREAM>(pl,             V2<T>::make(m[0].re, m[1].im));
+            stg2<T, STREAM>(pl + LINK_TILE, V2<T>::make(m[1].re, m[0].im));
         } else {
 #pragma unroll(UNR ? E : 1)
-            for (int e = 0; e < E; ++e) stg2<T, STREAM>(pl + (size_t)e * Vh + cb, V2<T>::make(m[e].re, m[e].im));
+            for (int e = 0; e < E; ++e) stg2<T, STREAM>(pl + e * LINK_TILE, V2<T>::make(m[e].re, m[e].im));
         }
     }
 };
@@ -196,6 +213,50 @@ template <int NC, class T, bool UNR> struct Mat {
                 for (int k = 0; k < NC; ++k) mad_cb(s, A[i * NC + k], B[j * NC + k]);
                 S[i * NC + j] = s;
             }
+    }
+    // S += (A B) C^dagger, one row of A B at a time: only B, C and S stay live across the rows, so the
+    // loads of all three operands can be issued before the first product.
+    // Same operation order per element as mul_nn followed by acc_nd.
+    static __device__ __forceinline__ void acc_nnd(C* S, const C* A, const C* B, const C* D) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i) {
+            C r[NC];
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad(s, A[i * NC + k], B[k * NC + j]);
+                r[j] = s;
+            }
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = S[i * NC + j];
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad_cb(s, r[k], D[j * NC + k]);
+                S[i * NC + j] = s;
+            }
+        }
+    }
+    // S += (A^dagger B) C, row by row; same operation order per element as mul_dn followed by acc_nn
+    static __device__ __forceinline__ void acc_dnn(C* S, const C* A, const C* B, const C* D) {
+#pragma unroll(UNR ? NC : 1)
+        for (int i = 0; i < NC; ++i) {
+            C r[NC];
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad_ca(s, A[k * NC + i], B[k * NC + j]);
+                r[j] = s;
+            }
+#pragma unroll(UNR ? NC : 1)
+            for (int j = 0; j < NC; ++j) {
+                C s = S[i * NC + j];
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad(s, r[k], D[k * NC + j]);
+                S[i * NC + j] = s;
+            }
+        }
     }
     // Re Tr (A B^dagger) = sum_ij Re(A_ij conj(B_ij))
     static __device__ __forceinline__ T retr_nd(const C* A, const C* B) {

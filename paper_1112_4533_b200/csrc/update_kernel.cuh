@@ -2,7 +2,7 @@
 // (parity, mu) sub-step of the sweep ("eight steps" per pass).
 //
 // One thread owns one link U_mu(x), x of the given parity. It gathers the 18 staple
-// links (eq 9) from the SoA planes with coalesced 64/128-bit loads, forms
+// links (eq 9) from the tiled SoA planes with coalesced 64/128-bit loads, forms
 // W = U S^dagger (step 2), runs the SU(2) subgroup loop (steps 3-5) and stores the link.
 //   UNR = true : matrices fully unrolled into registers (specialised SU(3)/SU(4))
 //   UNR = false: rolled loops over local arrays (generic SU(Nc))
@@ -61,7 +61,10 @@ __device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int 
     s.dm[3] = (t == 0) ? (g.L[3] - 1) * st : -st;
 }
 
-template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB>
+// FUSE3: each staple term S += A B C (three links) is evaluated row by row with all three operands
+// loaded up front (Mat::acc_nnd / acc_dnn): half as many load-wait phases per thread as the
+// two-step form (P = A B; S += P C), for the same registers. KUNR: unroll the loop over nu.
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, bool FUSE3 = false, bool KUNR = false>
 __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
     typedef LinkIO<NC, T, STORE, UNR> IO;
     typedef Mat<NC, T, UNR> M;
@@ -71,7 +74,6 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
     unsigned att_total = 0, exhausted = 0;
     if (active) {
         const int p = a.parity, mu = a.mu;
-        const unsigned Vh = a.g.Vh;
         SiteNbr s;
         site_of_thread(a.g, tix, p, s);
         const unsigned cb = s.cb;
@@ -80,37 +82,50 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
         C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
         M::zero(S);
         const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
-#pragma unroll 1
+#pragma unroll(KUNR ? 3 : 1)
         for (int k = 0; k < 3; ++k) {
             const int nu = k + (k >= mu ? 1 : 0);
             const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
             const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
             const typename IO::T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
             const typename IO::T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
-            // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
-            IO::template load<LD_RO>(pl_nu_s, Vh, cb, A);
-            IO::template load<LD_RO>(pl_mu_o, Vh, cb + (unsigned)dpnu, B);
-            M::mul_nn(A, B, P);
-            IO::template load<LD_RO>(pl_nu_o, Vh, cb + (unsigned)dpmu, A);
-            M::acc_nd(S, P, A);
-            // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
-            IO::template load<LD_RO>(pl_nu_o, Vh, cb + (unsigned)dmnu, A);
-            IO::template load<LD_RO>(pl_mu_o, Vh, cb + (unsigned)dmnu, B);
-            M::mul_dn(A, B, P);
-            IO::template load<LD_RO>(pl_nu_s, Vh, cb + (unsigned)(dmnu + dpmu), A);
-            M::acc_nn(S, P, A);
+            if (FUSE3) {
+                // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dpnu, B);
+                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dpmu, P);
+                IO::template load<LD_RO>(pl_nu_s, cb, A);
+                M::acc_nnd(S, A, B, P);
+                // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
+                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load<LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
+                M::acc_dnn(S, A, B, P);
+            } else {
+                // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+                IO::template load<LD_RO>(pl_nu_s, cb, A);
+                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dpnu, B);
+                M::mul_nn(A, B, P);
+                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dpmu, A);
+                M::acc_nd(S, P, A);
+                // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
+                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
+                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
+                M::mul_dn(A, B, P);
+                IO::template load<LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), A);
+                M::acc_nn(S, P, A);
+            }
         }
         typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
         C* U = A;
         C* W = B;
-        IO::template load<LD_STREAM>(pl_self, Vh, cb, U);
+        IO::template load<LD_STREAM>(pl_self, cb, U);
         M::mul_nd(U, S, W);                                   // W = U S^dagger
         update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex,
                                            a.sweep_ptr ? *a.sweep_ptr : a.sweep,
                                            pack_c2(0, (int)a.pass, p, mu, 0),
-                                           a.attempts ? a.attempts + cb : nullptr, (size_t)Vh,
+                                           a.attempts ? a.attempts + cb : nullptr, (size_t)a.g.Vh,
                                            att_total, exhausted);
-        IO::template store<true>(pl_self, Vh, cb, U);
+        IO::template store<true>(pl_self, cb, U);
     }
     if (KIND == KIND_HB) {
         for (int o = 16; o > 0; o >>= 1) {
@@ -129,9 +144,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
 // staple and update are quaternion arithmetic. Same algebra as the matrix path:
 // W = U S^bar, k = |W|, u~ = W/k, a = v u~^bar (heatbath, eq 14) or (u~^bar)^2 (eq 17), U' = a U.
 // ------------------------------------------------------------------------------------------
-template <class T, int LD> __device__ __forceinline__ void qload(const typename V2<T>::type* __restrict__ pl, unsigned Vh, unsigned cb, T q[4]) {
-    typename V2<T>::type v0 = ldg2<T, LD>(pl + cb);
-    typename V2<T>::type v1 = ldg2<T, LD>(pl + Vh + cb);
+template <class T> __device__ __forceinline__ size_t qsite(unsigned cb) {      // tiled layout, 2 pairs per link
+    return (size_t)(cb / LINK_TILE) * (2 * LINK_TILE) + (cb % LINK_TILE);
+}
+template <class T, int LD> __device__ __forceinline__ void qload(const typename V2<T>::type* __restrict__ pl, unsigned cb, T q[4]) {
+    pl += qsite<T>(cb);
+    typename V2<T>::type v0 = ldg2<T, LD>(pl);
+    typename V2<T>::type v1 = ldg2<T, LD>(pl + LINK_TILE);
     q[0] = v0.x; q[1] = v0.y; q[2] = v1.x; q[3] = v1.y;
 }
 template <class T> __device__ __forceinline__ void qconj(const T a[4], T o[4]) { o[0] = a[0]; o[1] = -a[1]; o[2] = -a[2]; o[3] = -a[3]; }
@@ -150,7 +169,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
         const unsigned cb = s.cb;
         const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
         const T2* base = (const T2*)a.links;
-        auto plane = [&](int d, int par) { return base + (size_t)(d * 2 + par) * 2 * Vh; };
+        auto plane = [&](int d, int par) { return base + (size_t)(d * 2 + par) * 2 * a.g.Vhp; };
         T S[4] = {0, 0, 0, 0}, A[4], B[4], Cq[4], P[4], Q[4];
         const T2* pl_mu_o = plane(mu, 1 - p);
 #pragma unroll
@@ -160,20 +179,20 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
             const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
             const T2* pl_nu_s = plane(nu, p);
             const T2* pl_nu_o = plane(nu, 1 - p);
-            qload<T, LD_RO>(pl_nu_s, Vh, cb, A);
-            qload<T, LD_RO>(pl_mu_o, Vh, cb + (unsigned)dpnu, B);
-            qload<T, LD_RO>(pl_nu_o, Vh, cb + (unsigned)dpmu, Cq);
+            qload<T, LD_RO>(pl_nu_s, cb, A);
+            qload<T, LD_RO>(pl_mu_o, cb + (unsigned)dpnu, B);
+            qload<T, LD_RO>(pl_nu_o, cb + (unsigned)dpmu, Cq);
             quat_mul(A, B, P); qconj(Cq, A); quat_mul(P, A, Q);
             S[0] += Q[0]; S[1] += Q[1]; S[2] += Q[2]; S[3] += Q[3];
-            qload<T, LD_RO>(pl_nu_o, Vh, cb + (unsigned)dmnu, A);
-            qload<T, LD_RO>(pl_mu_o, Vh, cb + (unsigned)dmnu, B);
-            qload<T, LD_RO>(pl_nu_s, Vh, cb + (unsigned)(dmnu + dpmu), Cq);
+            qload<T, LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
+            qload<T, LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
+            qload<T, LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), Cq);
             qconj(A, P); quat_mul(P, B, Q); quat_mul(Q, Cq, P);
             S[0] += P[0]; S[1] += P[1]; S[2] += P[2]; S[3] += P[3];
         }
-        T2* pl_self = (T2*)a.links + (size_t)(mu * 2 + p) * 2 * Vh;
+        T2* pl_self = (T2*)a.links + (size_t)(mu * 2 + p) * 2 * a.g.Vhp;
         T U[4], W[4], a4[4] = {1, 0, 0, 0};
-        qload<T, LD_STREAM>(pl_self, Vh, cb, U);
+        qload<T, LD_STREAM>(pl_self, cb, U);
         qconj(S, A);
         quat_mul(U, A, W);
         T k = Fn<T>::sqrt(W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
@@ -197,8 +216,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
         }
         if (ok) {
             quat_mul(a4, U, P);
-            stg2<T, true>(pl_self + cb, V2<T>::make(P[0], P[1]));
-            stg2<T, true>(pl_self + Vh + cb, V2<T>::make(P[2], P[3]));
+            T2* q = pl_self + qsite<T>(cb);
+            stg2<T, true>(q, V2<T>::make(P[0], P[1]));
+            stg2<T, true>(q + LINK_TILE, V2<T>::make(P[2], P[3]));
         }
     }
     if (KIND == KIND_HB) {

@@ -12,19 +12,64 @@ namespace sug {
 #define SUG_CAT_(a, b) a##b
 #define SUG_CAT(a, b) SUG_CAT_(a, b)
 
-// (HB_BLOCK, HB_MINB) and (OR_BLOCK, OR_MINB): threads per block and the __launch_bounds__ minimum
-// blocks per SM (= the register cap) of the heatbath and of the overrelaxation instantiation.
-template <int NC, class T, int STORE, bool UNR, int HB_BLOCK, int HB_MINB, int OR_BLOCK = HB_BLOCK, int OR_MINB = HB_MINB>
+// One launch configuration: threads per block, the __launch_bounds__ minimum blocks per SM (= the
+// register cap), and the kernel-structure switches of k_update (FUSE3, KUNR).
+template <int BLOCK_, int MINB_, bool FUSE3_ = false, bool KUNR_ = false> struct Cfg {
+    static constexpr int BLOCK = BLOCK_, MINB = MINB_;
+    static constexpr bool FUSE3 = FUSE3_, KUNR = KUNR_;
+};
+
+template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB>
 static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t st) {
     if (kind == KIND_HB) {
-        const unsigned grid = (a.g.Vh + HB_BLOCK - 1) / HB_BLOCK;
-        k_update<NC, T, STORE, KIND_HB, UNR, HB_BLOCK, HB_MINB><<<grid, HB_BLOCK, 0, st>>>(a);
+        const unsigned grid = (a.g.Vh + HB::BLOCK - 1) / HB::BLOCK;
+        k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR><<<grid, HB::BLOCK, 0, st>>>(a);
     } else {
-        const unsigned grid = (a.g.Vh + OR_BLOCK - 1) / OR_BLOCK;
-        k_update<NC, T, STORE, KIND_OR, UNR, OR_BLOCK, OR_MINB><<<grid, OR_BLOCK, 0, st>>>(a);
+        const unsigned grid = (a.g.Vh + OR::BLOCK - 1) / OR::BLOCK;
+        k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR><<<grid, OR::BLOCK, 0, st>>>(a);
     }
     return cudaGetLastError();
 }
+
+// Tuning overrides (-DSUG_CFG_...="Cfg<...>"), used only while sweeping on the GPU; the defaults below are
+// the measured choices (profiles/).
+#ifndef SUG_CFG_SU3_F64_HB
+#define SUG_CFG_SU3_F64_HB Cfg<256, 2>
+#endif
+#ifndef SUG_CFG_SU3_F64_OR
+#define SUG_CFG_SU3_F64_OR Cfg<128, 3, true, true>
+#endif
+#ifndef SUG_CFG_SU3_F32_HB
+#define SUG_CFG_SU3_F32_HB Cfg<128, 4>
+#endif
+#ifndef SUG_CFG_SU3_F32_OR
+#define SUG_CFG_SU3_F32_OR Cfg<128, 6>
+#endif
+#ifndef SUG_CFG_SU3R_F64_HB
+#define SUG_CFG_SU3R_F64_HB Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU3R_F64_OR
+#define SUG_CFG_SU3R_F64_OR Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU3R_F32_HB
+#define SUG_CFG_SU3R_F32_HB Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU3R_F32_OR
+#define SUG_CFG_SU3R_F32_OR Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU4_F64_HB
+#define SUG_CFG_SU4_F64_HB Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU4_F64_OR
+#define SUG_CFG_SU4_F64_OR Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU4_F32_HB
+#define SUG_CFG_SU4_F32_HB Cfg<128, 1>
+#endif
+#ifndef SUG_CFG_SU4_F32_OR
+#define SUG_CFG_SU4_F32_OR Cfg<128, 1>
+#endif
+typedef Cfg<64, 1> GenericCfg;   // rolled-loop generic kernel: local-memory arrays, small blocks
 
 cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateArgs& a, cudaStream_t st, uint64_t* n_launch) {
     constexpr int NC = SUG_NC;
@@ -38,32 +83,30 @@ cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateA
         else     { if (kind == KIND_HB) k_update_su2<float,  KIND_HB, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); else k_update_su2<float,  KIND_OR, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); }
         return cudaGetLastError();
     }
-    return f64 ? launch_update_t<NC, double, STORE_QUAT, false, 64, 1>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_QUAT, false, 64, 1>(kind, a, st);
+    return f64 ? launch_update_t<NC, double, STORE_QUAT, false, GenericCfg>(kind, a, st)
+               : launch_update_t<NC, float,  STORE_QUAT, false, GenericCfg>(kind, a, st);
 #elif SUG_NC == 3
     if (!v.generic) {
         if (v.store == STORE_RECON12)
-            return f64 ? launch_update_t<NC, double, STORE_RECON12, true, 128, 1>(kind, a, st)
-                       : launch_update_t<NC, float,  STORE_RECON12, true, 128, 1>(kind, a, st);
-        // measured on B200 at 48^4 (profiles/r01b_*): fp64 168 registers / 3 blocks beats both the
-        // spill-free 240 / 2 and the 128 / 4 build; fp32 fits 80 registers / 6 blocks without spills
-        return f64 ? launch_update_t<NC, double, STORE_FULL, true, 256, 2, 128, 3>(kind, a, st)
-                   : launch_update_t<NC, float,  STORE_FULL, true, 128, 4, 128, 6>(kind, a, st);
+            return f64 ? launch_update_t<NC, double, STORE_RECON12, true, SUG_CFG_SU3R_F64_HB, SUG_CFG_SU3R_F64_OR>(kind, a, st)
+                       : launch_update_t<NC, float,  STORE_RECON12, true, SUG_CFG_SU3R_F32_HB, SUG_CFG_SU3R_F32_OR>(kind, a, st);
+        return f64 ? launch_update_t<NC, double, STORE_FULL, true, SUG_CFG_SU3_F64_HB, SUG_CFG_SU3_F64_OR>(kind, a, st)
+                   : launch_update_t<NC, float,  STORE_FULL, true, SUG_CFG_SU3_F32_HB, SUG_CFG_SU3_F32_OR>(kind, a, st);
     }
     if (v.store == STORE_RECON12)
-        return f64 ? launch_update_t<NC, double, STORE_RECON12, false, 64, 1>(kind, a, st)
-                   : launch_update_t<NC, float,  STORE_RECON12, false, 64, 1>(kind, a, st);
-    return f64 ? launch_update_t<NC, double, STORE_FULL, false, 64, 1>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_FULL, false, 64, 1>(kind, a, st);
+        return f64 ? launch_update_t<NC, double, STORE_RECON12, false, GenericCfg>(kind, a, st)
+                   : launch_update_t<NC, float,  STORE_RECON12, false, GenericCfg>(kind, a, st);
+    return f64 ? launch_update_t<NC, double, STORE_FULL, false, GenericCfg>(kind, a, st)
+               : launch_update_t<NC, float,  STORE_FULL, false, GenericCfg>(kind, a, st);
 #elif SUG_NC == 4
     if (!v.generic)
-        return f64 ? launch_update_t<NC, double, STORE_FULL, true, 128, 1>(kind, a, st)
-                   : launch_update_t<NC, float,  STORE_FULL, true, 128, 1>(kind, a, st);
-    return f64 ? launch_update_t<NC, double, STORE_FULL, false, 64, 1>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_FULL, false, 64, 1>(kind, a, st);
+        return f64 ? launch_update_t<NC, double, STORE_FULL, true, SUG_CFG_SU4_F64_HB, SUG_CFG_SU4_F64_OR>(kind, a, st)
+                   : launch_update_t<NC, float,  STORE_FULL, true, SUG_CFG_SU4_F32_HB, SUG_CFG_SU4_F32_OR>(kind, a, st);
+    return f64 ? launch_update_t<NC, double, STORE_FULL, false, GenericCfg>(kind, a, st)
+               : launch_update_t<NC, float,  STORE_FULL, false, GenericCfg>(kind, a, st);
 #else
-    return f64 ? launch_update_t<NC, double, STORE_FULL, false, 64, 1>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_FULL, false, 64, 1>(kind, a, st);
+    return f64 ? launch_update_t<NC, double, STORE_FULL, false, GenericCfg>(kind, a, st)
+               : launch_update_t<NC, float,  STORE_FULL, false, GenericCfg>(kind, a, st);
 #endif
 }
 
