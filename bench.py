@@ -74,11 +74,16 @@ def measured_peaks():
 
 def ncu_traffic(tag):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
-        return json.load(open(p)).get(tag)
+        with open(p) as f:
+            for line in f.read().splitlines()[1:]:
+                t, b = line.split(",")[:2]
+                if t == tag:
+                    return float(b)
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
