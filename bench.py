@@ -132,12 +132,32 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def rank_seed(wl, rank):
+    """N > 1 runs independent replicas: rank r's Markov chain is seeded seed + r."""
+    return wl["seed"] + rank
+
+
+def max_over_ranks(dist, ms, device):
+    """The job's time is the slowest rank's device time (one all-reduce MAX of a double; gloo on CPU in tests)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world, updates_per_rank_step, ms, steps):
+    """value = the units ALL ranks processed / the max-over-ranks time"""
+    return world * updates_per_rank_step / (ms / steps * 1e-3)
+
+
 def make_lattice(su, wl, precision, recon12, kernel, rank, device):
     lat = su.Lattice(wl["Nc"], (wl["L"],) * 4, precision, recon12=recon12, kernel=kernel, device=device)
     if wl["start"] == "hot":
-        lat.init_hot(wl["seed"] + rank)
+        lat.init_hot(rank_seed(wl, rank))
     else:
-        lat.init_cold(wl["seed"] + rank)
+        lat.init_cold(rank_seed(wl, rank))
     return lat
 
 
@@ -293,7 +313,7 @@ def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
     Nc, V = wl["Nc"], wl["L"] ** 4
     updates_step = (N_HB + N_OR) * 4 * V
     t_step = res["ms"] / steps * 1e-3
-    value = n_ranks * updates_step / t_step
+    value = whole_job_rate(n_ranks, updates_step, res["ms"], steps)
     flops_step = 4 * V * (N_HB * flops_per_update(Nc, "hb", recon12) + N_OR * flops_per_update(Nc, "or", recon12))
     bpu = algorithmic_bytes_per_update(Nc, precision, recon12)
     tim = res["timing"]
@@ -351,10 +371,7 @@ def main():
     def timed(precision, r12, kernel, steps, wu, clocks):
         lat = make_lattice(su, wl, precision, r12, kernel, rank, local)
         res = time_resident(torch, dist, lat, wl, steps, wu, clocks, local)
-        if dist is not None:                   # max over ranks of the device time
-            t = torch.tensor([res["ms"]], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            res["ms"] = float(t.item())
+        res["ms"] = max_over_ranks(dist, res["ms"], "cuda")     # max over ranks of the device time
         return lat, res
 
     lat, res = timed(args.precision, recon12, args.kernel, args.steps, warmup, True)
@@ -362,11 +379,8 @@ def main():
     e2e = None
     if not args.no_e2e:
         r = time_e2e(torch, dist, lat, wl, max(1, args.e2e_steps))
-        if dist is not None:
-            t = torch.tensor([r["ms"]], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            r["ms"] = float(t.item())
-        e2e = {"value": world * (N_HB + N_OR) * 4 * wl["L"] ** 4 / (r["ms"] / r["steps"] * 1e-3), "unit": UNIT,
+        r["ms"] = max_over_ranks(dist, r["ms"], "cuda")
+        e2e = {"value": whole_job_rate(world, (N_HB + N_OR) * 4 * wl["L"] ** 4, r["ms"], r["steps"]), "unit": UNIT,
                "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"], "ms_per_step": r["ms"] / r["steps"],
                "steps": r["steps"], "what": "su_import_links(pinned host, canonical doubles) + step + su_export_links"}
     lat.close()
