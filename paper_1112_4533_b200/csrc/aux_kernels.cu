@@ -17,35 +17,55 @@ namespace sug {
 // Plaquette (eq 4): per site the six P_mu,nu; Re Tr P = Re Tr[(U_mu(x) U_nu(x+mu))
 // (U_nu(x) U_mu(x+nu))^dagger]. Products in T, site sum and reduction in double.
 // ------------------------------------------------------------------------------------------
+// Thread -> site: blocks alternate between the two parities of the same lattice region and walk it in the
+// update kernel's z-chunked order (site_of_thread), so a link is fetched from DRAM once: it is read as
+// "own" link by its site and as forward neighbour by three sites of the other parity in the same or the
+// next chunk, all while it is still in L2.
 template <int NC, class T, int STORE, bool UNR>
-__global__ void __launch_bounds__(REDUCE_BLOCK) k_plaquette(const AuxArgs a) {
+__global__ void __launch_bounds__(PLAQ_BLOCK, PLAQ_MINB) k_plaquette(const AuxArgs a) {
     typedef LinkIO<NC, T, STORE, UNR> IO;
     typedef Mat<NC, T, UNR> M;
     typedef cx<T> C;
-    const unsigned idx = blockIdx.x * REDUCE_BLOCK + threadIdx.x;
+    const int p = (int)(blockIdx.x & 1u);
+    const unsigned tix = (blockIdx.x >> 1) * PLAQ_BLOCK + threadIdx.x;
     double acc = 0.0;
-    if (idx < 2u * a.g.Vh) {
-        const unsigned Vh = a.g.Vh;
-        const int p = idx >= Vh ? 1 : 0;
-        const unsigned cb = idx - (p ? Vh : 0u);
-        int c[4];
-        decode_cb(a.g, cb, p, c);
-        unsigned fwd[4];
+    if (tix < a.g.Vh) {
+        SiteNbr s;
+        site_of_thread(a.g, tix, p, s);
+        const unsigned cb = s.cb;
+        if (UNR && NC <= 3) {
+            // the site's four links stay in registers; each of the 6 plaquettes adds two neighbour loads
+            C Uo[4][NC * NC], B[NC * NC], D[NC * NC], P[NC * NC], Q[NC * NC];
 #pragma unroll
-        for (int d = 0; d < 4; ++d) fwd[d] = cb_shift(a.g, c, d, +1);
-        C A[NC * NC], B[NC * NC], P[NC * NC], Q[NC * NC];
+            for (int d = 0; d < 4; ++d) IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, d, p), cb, Uo[d]);
+#pragma unroll
+            for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+                for (int nu = mu + 1; nu < 4; ++nu) {
+                    IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, 1 - p), cb + (unsigned)s.dp[mu], B);
+                    IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, 1 - p), cb + (unsigned)s.dp[nu], D);
+                    M::mul_nn(Uo[mu], B, P);
+                    M::mul_nn(Uo[nu], D, Q);
+                    acc += (double)M::retr_nd(P, Q);
+                }
+        } else {
+            // Nc >= 4: four resident links would not fit the register file; two loads per product instead
+            C A[NC * NC], B[NC * NC], P[NC * NC], Q[NC * NC];
 #pragma unroll 1
-        for (int mu = 0; mu < 3; ++mu)
+            for (int mu = 0; mu < 3; ++mu)
 #pragma unroll 1
-            for (int nu = mu + 1; nu < 4; ++nu) {
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, p), cb, A);
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, 1 - p), fwd[mu], B);
-                M::mul_nn(A, B, P);
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, p), cb, A);
-                IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, 1 - p), fwd[nu], B);
-                M::mul_nn(A, B, Q);
-                acc += (double)M::retr_nd(P, Q);
-            }
+                for (int nu = mu + 1; nu < 4; ++nu) {
+                    const unsigned fmu = cb + (unsigned)sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+                    const unsigned fnu = cb + (unsigned)sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+                    IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, p), cb, A);
+                    IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, 1 - p), fmu, B);
+                    M::mul_nn(A, B, P);
+                    IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, nu, p), cb, A);
+                    IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, mu, 1 - p), fnu, B);
+                    M::mul_nn(A, B, Q);
+                    acc += (double)M::retr_nd(P, Q);
+                }
+        }
     }
     acc = block_sum(acc);
     if (threadIdx.x == 0) a.partials[blockIdx.x] = acc;
@@ -97,21 +117,36 @@ static __global__ void __launch_bounds__(REDUCE_BLOCK) k_reduce_final(const doub
 // Gram-Schmidt / determinant on a local matrix (rolled loops), used by reunitarise (Nc >= 4)
 // and by the hot start (always double, reading R20).
 // ------------------------------------------------------------------------------------------
-template <int NC, class R>
-__device__ void gram_schmidt_rows(cx<R>* U, int nrows) {
-#pragma unroll 1
-    for (int r = 0; r < nrows; ++r) {
-#pragma unroll 1
+template <int NC, class R, bool UNR = false>
+__device__ __forceinline__ void gram_schmidt_rows(cx<R>* U, int nrows) {
+#pragma unroll(UNR ? NC : 1)
+    for (int r = 0; r < (UNR ? NC : nrows); ++r) {
+#pragma unroll(UNR ? NC : 1)
         for (int p = 0; p < r; ++p) {
             cx<R> dot = mk<R>(0, 0);
+#pragma unroll(UNR ? NC : 1)
             for (int k = 0; k < NC; ++k) mad_ca(dot, U[p * NC + k], U[r * NC + k]);
+#pragma unroll(UNR ? NC : 1)
             for (int k = 0; k < NC; ++k) U[r * NC + k] = U[r * NC + k] - dot * U[p * NC + k];
         }
         R n2 = 0;
+#pragma unroll(UNR ? NC : 1)
         for (int k = 0; k < NC; ++k) n2 += U[r * NC + k].re * U[r * NC + k].re + U[r * NC + k].im * U[r * NC + k].im;
         R inv = (R)1 / Fn<R>::sqrt(n2);
+#pragma unroll(UNR ? NC : 1)
         for (int k = 0; k < NC; ++k) U[r * NC + k] = inv * U[r * NC + k];
     }
+}
+
+// det of a 4x4 complex matrix by the 2x2-minor (Laplace) expansion over rows {0,1} x {2,3}: no pivoting,
+// no dynamic indexing, so it stays in registers (used for the phase conj(det)/|det| only).
+template <class R>
+__device__ __forceinline__ cx<R> determinant4(const cx<R>* A) {
+    const cx<R> s0 = A[0] * A[5] - A[1] * A[4], s1 = A[0] * A[6] - A[2] * A[4], s2 = A[0] * A[7] - A[3] * A[4];
+    const cx<R> s3 = A[1] * A[6] - A[2] * A[5], s4 = A[1] * A[7] - A[3] * A[5], s5 = A[2] * A[7] - A[3] * A[6];
+    const cx<R> c5 = A[10] * A[15] - A[11] * A[14], c4 = A[9] * A[15] - A[11] * A[13], c3 = A[9] * A[14] - A[10] * A[13];
+    const cx<R> c2 = A[8] * A[15] - A[11] * A[12], c1 = A[8] * A[14] - A[10] * A[12], c0 = A[8] * A[13] - A[9] * A[12];
+    return (s0 * c5 - s1 * c4) + (s2 * c3 + s3 * c2) + (s5 * c0 - s4 * c1);
 }
 
 template <int NC, class R>
@@ -160,27 +195,56 @@ __device__ __forceinline__ bool link_of_thread(const Geom& g, unsigned idx, int&
     return true;
 }
 
-// Reunitarisation (reading R10), arithmetic in T.
+// SU(3) rows 0,1 by modified Gram-Schmidt in registers (same operation order as gram_schmidt_rows)
+template <class T>
+__device__ __forceinline__ void gram_schmidt_su3_two_rows(cx<T>* U) {
+    T n2 = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) n2 += U[k].re * U[k].re + U[k].im * U[k].im;
+    T inv = (T)1 / Fn<T>::sqrt(n2);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) U[k] = inv * U[k];
+    cx<T> dot = mk<T>(0, 0);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) mad_ca(dot, U[k], U[3 + k]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) U[3 + k] = U[3 + k] - dot * U[k];
+    n2 = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) n2 += U[3 + k].re * U[3 + k].re + U[3 + k].im * U[3 + k].im;
+    inv = (T)1 / Fn<T>::sqrt(n2);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) U[3 + k] = inv * U[3 + k];
+}
+
+// Reunitarisation (reading R10), arithmetic in T. Nc <= 4 runs in registers.
 template <int NC, class T, int STORE, bool UNR>
 __global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
-    typedef LinkIO<NC, T, STORE, UNR> IO;
+    typedef LinkIO<NC, T, STORE, (NC <= 4)> IO;
     int mu, p; unsigned cb;
     if (!link_of_thread(a.g, blockIdx.x * 128u + threadIdx.x, mu, p, cb)) return;
     typename IO::T2* pl = IO::plane(a.links, a.g, mu, p);
     cx<T> U[NC * NC];
-    IO::template load<LD_PLAIN>(pl, cb, U);
+    IO::template load<LD_STREAM>(pl, cb, U);
     if (NC == 2) {
         T n = Fn<T>::sqrt((U[0].re * U[0].re + U[0].im * U[0].im) + (U[1].re * U[1].re + U[1].im * U[1].im));
         U[0] = mk<T>(U[0].re / n, U[0].im / n);
         U[1] = mk<T>(U[1].re / n, U[1].im / n);
     } else if (NC == 3) {
-        gram_schmidt_rows<NC, T>(U, 2);
+        gram_schmidt_su3_two_rows<T>(U);
         su3_third_row(U);
+    } else if (NC == 4) {
+        gram_schmidt_rows<NC, T, true>(U, NC);
+        const cx<T> d = determinant4<T>(U);
+        const T inv = (T)1 / Fn<T>::sqrt(d.re * d.re + d.im * d.im);
+        const cx<T> ph = mk<T>(d.re * inv, -d.im * inv);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) U[(NC - 1) * NC + k] = U[(NC - 1) * NC + k] * ph;
     } else {
         gram_schmidt_rows<NC, T>(U, NC);
         fix_determinant_phase<NC, T>(U);
     }
-    IO::store(pl, cb, U);
+    IO::template store<true>(pl, cb, U);
 }
 
 template <int NC, class T, int STORE, bool UNR>
@@ -318,8 +382,8 @@ __global__ void __launch_bounds__(128) k_import(const AuxArgs a) {
     } while (0)
 
 cudaError_t SUG_CAT(plaquette_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
-    const unsigned nb = reduce_blocks(2u * a.g.Vh);
-    SUG_MEAS_DISPATCH(k_plaquette, nb, REDUCE_BLOCK);
+    const unsigned nb = plaquette_blocks(a.g.Vh);
+    SUG_MEAS_DISPATCH(k_plaquette, nb, PLAQ_BLOCK);
     const double scale = 1.0 / (6.0 * 2.0 * (double)a.g.Vh * (double)SUG_NC);
     k_reduce_final<<<1, REDUCE_BLOCK, 0, st>>>(a.partials, nb, 1, scale, a.result);
     ++*n_launch;

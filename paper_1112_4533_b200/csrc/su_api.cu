@@ -3,6 +3,7 @@
 // of update_kernels.cu / aux_kernels.cu; nothing here falls back to the CPU.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <new>
@@ -49,6 +50,10 @@ struct su_lattice {
 
 namespace {
 
+#ifndef SUG_ZCHUNK_MB
+#define SUG_ZCHUNK_MB 16
+#endif
+
 const char* kNullHandle = "null lattice handle";
 
 struct DeviceGuard {
@@ -91,9 +96,14 @@ size_t plane_sites(size_t Vh) { return (Vh + LINK_TILE - 1) / LINK_TILE * LINK_T
 // of the algorithmic bytes (profiles/r01a, r01b).
 int traversal_z_chunk(const Geom& g, size_t link_bytes) {
     const size_t plane = (size_t)g.L[0] * g.L[1] * 4 * link_bytes;   // one z-plane of one time slice, 4 directions
+    size_t limit = (size_t)SUG_ZCHUNK_MB << 20;
+    if (const char* e = getenv("SU_GAUGE_ZCHUNK_MB")) {              // tuning knob
+        const long v = atol(e);
+        if (v > 0) limit = (size_t)v << 20;
+    }
     int zc = 1;
     for (int d = 1; d <= g.L[2]; ++d)
-        if (g.L[2] % d == 0 && plane * (size_t)d <= ((size_t)16 << 20)) zc = d;
+        if (g.L[2] % d == 0 && plane * (size_t)d <= limit) zc = d;
     return zc;
 }
 
@@ -254,7 +264,7 @@ su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precis
         h->owns_links = (st == SU_OK);
     }
     const unsigned Vs = (unsigned)Lx * Ly * Lz;
-    const size_t npart = (size_t)reduce_blocks(2u * h->g.Vh) + 2 * (size_t)reduce_blocks(Vs) + 2;
+    const size_t npart = (size_t)plaquette_blocks(h->g.Vh) + 2 * (size_t)reduce_blocks(Vs) + 2;
     if (st == SU_OK && cudaMalloc(&h->d_partials, npart * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_result, 2 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_counters, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ENOMEM;

@@ -12,6 +12,9 @@ enum : int { STORE_FULL = 0, STORE_RECON12 = 1, STORE_QUAT = 2 };
 enum : int { KIND_HB = 0, KIND_OR = 1 };
 enum : int { RNG_KP = 0, RNG_DIR = 1, RNG_HOT = 2 };
 constexpr int KP_MAX_ATTEMPTS = 1024;   // reading R15
+#ifndef SUG_KP_PRETEST
+#define SUG_KP_PRETEST 1
+#endif
 
 template <class T> struct V2;
 template <> struct V2<float>  { typedef float2  type; static __device__ __forceinline__ float2  make(float a, float b)   { return make_float2(a, b); } };
@@ -301,7 +304,11 @@ template <> struct Fn<float> {
     static __device__ __forceinline__ float log(float x) { return logf(x); }
     static __device__ __forceinline__ float cos(float x) { return cosf(x); }
     static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
+    static __device__ __forceinline__ float rsqrt(float x) { return rsqrtf(x); }
     static __device__ __forceinline__ void sincos(float x, float* s, float* c) { sincosf(x, s, c); }
+    // cos / sincos of 2 pi u for u in (0,1]: the pi-scaled forms need no range reduction of an irrational multiple
+    static __device__ __forceinline__ float cos2pi(float u) { return cospif(2.0f * u); }
+    static __device__ __forceinline__ void sincos2pi(float u, float* s, float* c) { sincospif(2.0f * u, s, c); }
     static __device__ __forceinline__ float max0(float x) { return fmaxf(x, 0.0f); }
     static __device__ __forceinline__ bool finite(float x) { return isfinite(x); }
 };
@@ -309,38 +316,70 @@ template <> struct Fn<double> {
     static __device__ __forceinline__ double log(double x) { return ::log(x); }
     static __device__ __forceinline__ double cos(double x) { return ::cos(x); }
     static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+    static __device__ __forceinline__ double rsqrt(double x) { return ::rsqrt(x); }
     static __device__ __forceinline__ void sincos(double x, double* s, double* c) { ::sincos(x, s, c); }
+    static __device__ __forceinline__ double cos2pi(double u) { return ::cospi(2.0 * u); }
+    static __device__ __forceinline__ void sincos2pi(double u, double* s, double* c) { ::sincospi(2.0 * u, s, c); }
     static __device__ __forceinline__ double max0(double x) { return fmax(x, 0.0); }
     static __device__ __forceinline__ bool finite(double x) { return isfinite(x); }
 };
 
 // Kennedy-Pendleton draw of v = (a0, a): P(a0) ~ sqrt(1-a0^2) exp(alpha a0) (eq 13),
 // a uniform on the sphere of radius sqrt(1-a0^2). Returns attempts used, 0 = none.
+// m_inv2a = -1 / (2 alpha), supplied by the caller (it has 1/k already).
+//
+// fp64: the accept test r4^2 <= 1 - lambda^2  <=>  M = 2 alpha (1 - r4^2) + ln r1 + cos^2(2 pi r2) ln r3 >= 0
+// is first evaluated in fp32 with the SFU approximations (|error of M| < 1e-4 + 2 alpha 5e-7). Only when
+// |M| is inside a 10x wider band is the decision taken with the exact fp64 expression, so the decision is
+// always the fp64 one, and the accepted attempt's lambda^2 is then evaluated in fp64 once, after the
+// loop, by the whole warp together (a warp would otherwise run the fp64 log/log/cos body for every
+// attempt any of its lanes needs: 1.9 times per draw at beta = 6 instead of once).
 template <class T>
-__device__ __forceinline__ int kp_draw(T alpha, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
+__device__ __forceinline__ int kp_draw(T alpha, T m_inv2a, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
                                        uint32_t c2_base, T v[4]) {
-    const T TWO_PI = (T)6.283185307179586476925286766559;
     if (!(alpha > (T)0) || !Fn<T>::finite(alpha)) return 0;
-    const T inv2a = (T)2 * alpha;
+    constexpr bool PRETEST = (sizeof(T) == 8) && (SUG_KP_PRETEST != 0);
+    const float two_af = 2.0f * (float)alpha;
+    const float band = 1e-3f + two_af * 4e-6f;
     T a0 = 0;
     int used = 0;
+    uint32_t w[4];
+    // lanes leave the accept loop after different numbers of attempts; without an explicit barrier the
+    // compiler lets every exit group run the rest of the draw on its own (ncu: the direction part ran 1.6x
+    // per warp). The mask is the set of lanes converged here, so the barrier is safe in a ragged last warp.
+    const unsigned converged = __activemask();
     for (int n = 0; n < KP_MAX_ATTEMPTS; ++n) {
-        uint32_t w[4];
         philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_KP << 28), (uint32_t)n, k0, k1, w);
+        if (PRETEST) {
+            const float S = 2.3283064365386963e-10f;      // 2^-32
+            const float r1f = (__uint2float_rn(w[0]) + 1.0f) * S, r2f = (__uint2float_rn(w[1]) + 1.0f) * S;
+            const float r3f = (__uint2float_rn(w[2]) + 1.0f) * S, r4f = (__uint2float_rn(w[3]) + 1.0f) * S;
+            const float cf = __cosf(6.2831853071795865f * r2f);
+            const float M = two_af * (1.0f - r4f * r4f) + (__logf(r1f) + cf * cf * __logf(r3f));
+            if (M > band) { used = n + 1; break; }
+            if (M < -band) continue;
+        }
         T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]), r4 = uniform01<T>(w[3]);
-        T c = Fn<T>::cos(TWO_PI * r2);
-        T lambda2 = -(Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) / inv2a;
+        T c = Fn<T>::cos2pi(r2);
+        T lambda2 = (Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) * m_inv2a;
         if (r4 * r4 <= (T)1 - lambda2) { a0 = (T)1 - (T)2 * lambda2; used = n + 1; break; }
     }
+    __syncwarp(converged);
     if (!used) return 0;
-    uint32_t w[4];
-    philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_DIR << 28), 0u, k0, k1, w);
-    T u1 = uniform01<T>(w[0]), u2 = uniform01<T>(w[1]);
+    if (PRETEST) {
+        T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]);
+        T c = Fn<T>::cos2pi(r2);
+        T lambda2 = (Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) * m_inv2a;
+        a0 = (T)1 - (T)2 * lambda2;
+    }
+    uint32_t d[4];
+    philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_DIR << 28), 0u, k0, k1, d);
+    T u1 = uniform01<T>(d[0]), u2 = uniform01<T>(d[1]);
     T cos_t = (T)1 - (T)2 * u1;
     T sin_t = Fn<T>::sqrt(Fn<T>::max0((T)1 - cos_t * cos_t));
     T rho = Fn<T>::sqrt(Fn<T>::max0((T)1 - a0 * a0));
     T sp, cp;
-    Fn<T>::sincos(TWO_PI * u2, &sp, &cp);
+    Fn<T>::sincos2pi(u2, &sp, &cp);
     v[0] = a0; v[1] = rho * sin_t * cp; v[2] = rho * sin_t * sp; v[3] = rho * cos_t;
     return used;
 }
@@ -365,6 +404,8 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                                                  uint8_t* att_out, size_t att_stride,
                                                  unsigned& att_total, unsigned& exhausted) {
     int q = 0;
+    const T two_beta_over_nc = (T)2 * beta / (T)NC;      // alpha = 2 beta k / Nc (reading R3)
+    const T m_nc_over_4beta = (T)-0.25 * (T)NC / beta;   // -1 / (2 alpha) = this / k   (heatbath only)
 #pragma unroll(UNR ? NC : 1)
     for (int i = 0; i < NC - 1; ++i) {
 #pragma unroll(UNR ? NC : 1)
@@ -372,18 +413,23 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
             const cx<T> wii = W[i * NC + i], wij = W[i * NC + j], wji = W[j * NC + i], wjj = W[j * NC + j];
             T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
             T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
-            T k = Fn<T>::sqrt(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
-            bool ok = (k > (T)0) && Fn<T>::finite(k);
+            const T n2 = r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3;          // k^2
+            bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
             T a[4] = {(T)1, (T)0, (T)0, (T)0};
             int used = 0;
             if (ok) {
-                T ud[4] = {r0 / k, -r1 / k, -r2 / k, -r3 / k};
                 if (KIND == KIND_HB) {
+                    const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;          // 1/k and k without a division
+                    T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                     T v[4];
-                    used = kp_draw<T>((T)2 * beta * k / (T)NC, k0, k1, c0, c1, c2_base | (uint32_t)q, v);
+                    used = kp_draw<T>(two_beta_over_nc * k, m_nc_over_4beta * ik, k0, k1, c0, c1,
+                                      c2_base | (uint32_t)q, v);
                     if (used) quat_mul(v, ud, a); else ok = false;
                 } else {
-                    quat_mul(ud, ud, a);
+                    // a = (u~^dagger)^2 = conj(r)^2 / k^2 (eq 17): no square root, one reciprocal
+                    const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
+                    a[0] = (r0 * r0 - (r1 * r1 + r2 * r2 + r3 * r3)) * in2;
+                    a[1] = m2r0 * r1; a[2] = m2r0 * r2; a[3] = m2r0 * r3;
                 }
             }
             if (KIND == KIND_HB) {

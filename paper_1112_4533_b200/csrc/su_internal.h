@@ -47,5 +47,10 @@ SUG_DECLARE_NC(8)
 
 constexpr int REDUCE_BLOCK = 256;
 inline unsigned reduce_blocks(unsigned n) { return (n + REDUCE_BLOCK - 1) / REDUCE_BLOCK; }
+constexpr int PLAQ_BLOCK = 128;          // plaquette kernel: blocks alternate parity over the same region
+#ifndef PLAQ_MINB
+#define PLAQ_MINB 3
+#endif
+inline unsigned plaquette_blocks(unsigned Vh) { return 2u * ((Vh + PLAQ_BLOCK - 1) / PLAQ_BLOCK); }
 
 }  // namespace sug

@@ -195,18 +195,22 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
         qload<T, LD_STREAM>(pl_self, cb, U);
         qconj(S, A);
         quat_mul(U, A, W);
-        T k = Fn<T>::sqrt(W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
-        bool ok = (k > (T)0) && Fn<T>::finite(k);
+        const T n2 = W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3];      // k^2
+        bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
         int used = 0;
         if (ok) {
-            T ud[4] = {W[0] / k, -W[1] / k, -W[2] / k, -W[3] / k};
             if (KIND == KIND_HB) {
+                const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;
+                T ud[4] = {W[0] * ik, -W[1] * ik, -W[2] * ik, -W[3] * ik};
                 T v[4];
-                used = kp_draw<T>((T)a.beta * k, a.k0, a.k1, s.lex, a.sweep_ptr ? *a.sweep_ptr : a.sweep,
+                used = kp_draw<T>((T)a.beta * k, (T)-0.5 / (T)a.beta * ik, a.k0, a.k1, s.lex, a.sweep_ptr ? *a.sweep_ptr : a.sweep,
                                   pack_c2(0, (int)a.pass, p, mu, 0), v);
                 if (used) quat_mul(v, ud, a4); else ok = false;
             } else {
-                quat_mul(ud, ud, a4);
+                // a = conj(W)^2 / k^2 (eq 17)
+                const T in2 = (T)1 / n2, m2w0 = (T)-2 * W[0] * in2;
+                a4[0] = (W[0] * W[0] - (W[1] * W[1] + W[2] * W[2] + W[3] * W[3])) * in2;
+                a4[1] = m2w0 * W[1]; a4[2] = m2w0 * W[2]; a4[3] = m2w0 * W[3];
             }
         }
         if (KIND == KIND_HB) {

@@ -2,6 +2,7 @@
 // (update_kernel.cuh) for one (parity, mu) sub-step. Compiled once per colour count with
 // -DSUG_NC=<Nc>. Block size / minimum blocks per SM per variant: DESIGN.md "Launch configuration".
 #include "su_internal.h"
+#include "update_rows_kernel.cuh"
 
 #ifndef SUG_NC
 #error "compile with -DSUG_NC=<Nc>"
@@ -34,42 +35,44 @@ static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t s
 // Tuning overrides (-DSUG_CFG_...="Cfg<...>"), used only while sweeping on the GPU; the defaults below are
 // the measured choices (profiles/).
 #ifndef SUG_CFG_SU3_F64_HB
-#define SUG_CFG_SU3_F64_HB Cfg<256, 2>
+#define SUG_CFG_SU3_F64_HB Cfg<128, 3, true, true>
 #endif
 #ifndef SUG_CFG_SU3_F64_OR
 #define SUG_CFG_SU3_F64_OR Cfg<128, 3, true, true>
 #endif
 #ifndef SUG_CFG_SU3_F32_HB
-#define SUG_CFG_SU3_F32_HB Cfg<128, 4>
+#define SUG_CFG_SU3_F32_HB Cfg<128, 4, true, true>
 #endif
 #ifndef SUG_CFG_SU3_F32_OR
-#define SUG_CFG_SU3_F32_OR Cfg<128, 6>
+#define SUG_CFG_SU3_F32_OR Cfg<128, 5, true, true>
 #endif
 #ifndef SUG_CFG_SU3R_F64_HB
-#define SUG_CFG_SU3R_F64_HB Cfg<128, 1>
+#define SUG_CFG_SU3R_F64_HB Cfg<128, 3, true, true>
 #endif
 #ifndef SUG_CFG_SU3R_F64_OR
-#define SUG_CFG_SU3R_F64_OR Cfg<128, 1>
+#define SUG_CFG_SU3R_F64_OR Cfg<128, 3, true, true>
 #endif
 #ifndef SUG_CFG_SU3R_F32_HB
 #define SUG_CFG_SU3R_F32_HB Cfg<128, 1>
 #endif
 #ifndef SUG_CFG_SU3R_F32_OR
-#define SUG_CFG_SU3R_F32_OR Cfg<128, 1>
+#define SUG_CFG_SU3R_F32_OR Cfg<128, 3, true, true>
 #endif
 #ifndef SUG_CFG_SU4_F64_HB
 #define SUG_CFG_SU4_F64_HB Cfg<128, 1>
 #endif
 #ifndef SUG_CFG_SU4_F64_OR
-#define SUG_CFG_SU4_F64_OR Cfg<128, 1>
+#define SUG_CFG_SU4_F64_OR Cfg<128, 2, true, true>
 #endif
 #ifndef SUG_CFG_SU4_F32_HB
-#define SUG_CFG_SU4_F32_HB Cfg<128, 1>
+#define SUG_CFG_SU4_F32_HB Cfg<128, 3, true, true>
 #endif
 #ifndef SUG_CFG_SU4_F32_OR
-#define SUG_CFG_SU4_F32_OR Cfg<128, 1>
+#define SUG_CFG_SU4_F32_OR Cfg<128, 3, true, true>
 #endif
-typedef Cfg<64, 1> GenericCfg;   // rolled-loop generic kernel: local-memory arrays, small blocks
+// Generic SU(Nc): the row-per-lane kernel (update_rows_kernel.cuh) for full Nc x Nc storage; the rolled-loop
+// thread-per-link form (local-memory arrays, small blocks) only for the SU(2) quaternion / SU(3) two-row layouts.
+typedef Cfg<64, 1> GenericCfg;
 
 cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateArgs& a, cudaStream_t st, uint64_t* n_launch) {
     constexpr int NC = SUG_NC;
@@ -96,17 +99,14 @@ cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateA
     if (v.store == STORE_RECON12)
         return f64 ? launch_update_t<NC, double, STORE_RECON12, false, GenericCfg>(kind, a, st)
                    : launch_update_t<NC, float,  STORE_RECON12, false, GenericCfg>(kind, a, st);
-    return f64 ? launch_update_t<NC, double, STORE_FULL, false, GenericCfg>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_FULL, false, GenericCfg>(kind, a, st);
+    return f64 ? launch_update_rows<NC, double>(kind, a, st) : launch_update_rows<NC, float>(kind, a, st);
 #elif SUG_NC == 4
     if (!v.generic)
         return f64 ? launch_update_t<NC, double, STORE_FULL, true, SUG_CFG_SU4_F64_HB, SUG_CFG_SU4_F64_OR>(kind, a, st)
                    : launch_update_t<NC, float,  STORE_FULL, true, SUG_CFG_SU4_F32_HB, SUG_CFG_SU4_F32_OR>(kind, a, st);
-    return f64 ? launch_update_t<NC, double, STORE_FULL, false, GenericCfg>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_FULL, false, GenericCfg>(kind, a, st);
+    return f64 ? launch_update_rows<NC, double>(kind, a, st) : launch_update_rows<NC, float>(kind, a, st);
 #else
-    return f64 ? launch_update_t<NC, double, STORE_FULL, false, GenericCfg>(kind, a, st)
-               : launch_update_t<NC, float,  STORE_FULL, false, GenericCfg>(kind, a, st);
+    return f64 ? launch_update_rows<NC, double>(kind, a, st) : launch_update_rows<NC, float>(kind, a, st);
 #endif
 }
 

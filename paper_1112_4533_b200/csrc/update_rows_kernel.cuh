@@ -1,0 +1,237 @@
+// update_rows_kernel.cuh — the GENERIC SU(Nc) staple + link-update kernel:
+// any Nc, nothing specialised per group, full Nc x Nc storage.
+//
+// The paper's generic kernel gives one thread a whole link and keeps its Nc x Nc matrices in local
+// memory; its cost explodes with Nc ("SU(6) ~ 10x optimised SU(3)"). Here a link is
+// updated by a group of Nc lanes of one warp, lane r owning ROW r of every matrix in registers:
+//   staple term  S_r += (A_r . B) . C^dagger         A_r in registers, B and C staged in shared memory
+//                S_r += (A^dagger B)_r . C           A, B, C staged in shared memory
+//   W_r = U_r . S^dagger                             S staged in shared memory
+//   subgroup (i,j): lanes i and j exchange rows by warp shuffle, every lane of the group evaluates
+//                   the 2x2 projection and the Kennedy-Pendleton draw redundantly (no extra cost in
+//                   SIMT: the lanes would idle otherwise), rows i and j are rotated (eq 15).
+// A warp holds floor(32 / Nc) links; left-over lanes shadow the last group and never store.
+// The order of operations inside every sum is the one of update_kernel.cuh and of the oracle.
+#pragma once
+#include "update_kernel.cuh"
+
+namespace sug {
+
+template <int NC> struct RowsCfg {
+    static constexpr int LPW = 32 / NC;                       // links per warp
+    static constexpr int STRIDE = NC * NC + 1;                // complex elements per staged matrix (+1: bank spread)
+    static constexpr int NBUF = 5;                            // upper term: B, C; lower term: A, B, C
+    static constexpr size_t bytes(int w, size_t real) { return (size_t)w * LPW * NBUF * STRIDE * 2 * real; }
+};
+// warps per block: as many (<= 4) as keep the staging area within 48 KB of static shared memory
+template <int NC, class T> struct RowsWarps {
+    static constexpr size_t LIM = 48 * 1024, R = sizeof(T);
+    static constexpr int value = RowsCfg<NC>::bytes(4, R) <= LIM ? 4 : (RowsCfg<NC>::bytes(3, R) <= LIM ? 3 : (RowsCfg<NC>::bytes(2, R) <= LIM ? 2 : 1));
+};
+
+template <class T> __device__ __forceinline__ cx<T> shfl_cx(cx<T> v, int src) {
+    return mk<T>(__shfl_sync(0xffffffffu, v.re, src), __shfl_sync(0xffffffffu, v.im, src));
+}
+// element `idx` of a register-resident row without dynamic indexing
+template <int NC, class T> __device__ __forceinline__ cx<T> row_pick(const cx<T>* row, int idx) {
+    cx<T> v = row[0];
+#pragma unroll
+    for (int c = 1; c < NC; ++c) if (idx == c) v = row[c];
+    return v;
+}
+
+template <int NC, class T, int KIND>
+__global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value) k_update_rows(const UpdateArgs a) {
+    typedef RowsCfg<NC> Cfg;
+    typedef LinkIO<NC, T, STORE_FULL, true> IO;
+    typedef typename IO::T2 T2;
+    typedef cx<T> C;
+    constexpr int WARPS = RowsWarps<NC, T>::value;
+    constexpr int LPW = Cfg::LPW, STRIDE = Cfg::STRIDE;
+    __shared__ C stage[WARPS * LPW][Cfg::NBUF][STRIDE];
+
+    const int lane = (int)(threadIdx.x & 31u), warp = (int)(threadIdx.x >> 5);
+    const bool shadow = lane >= LPW * NC;                     // left-over lanes repeat the last group's work
+    const int g = shadow ? LPW - 1 : lane / NC;               // link slot in the warp
+    const int r = shadow ? lane - LPW * NC : lane - g * NC;   // row owned by this lane
+    const int gbase = g * NC;                                 // first lane of the group
+    unsigned tix = (blockIdx.x * WARPS + (unsigned)warp) * LPW + (unsigned)g;
+    const bool owner = !shadow && tix < a.g.Vh;               // lanes past the end redo the last link, never store
+    if (tix >= a.g.Vh) tix = a.g.Vh - 1;
+    C(*M)[STRIDE] = stage[warp * LPW + g];
+
+    const int p = a.parity, mu = a.mu;
+    SiteNbr s;
+    site_of_thread(a.g, tix, p, s);
+    const unsigned cb = s.cb;
+    const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+
+    // row r of a link straight from the tiled SoA plane
+    auto load_row = [&](const T2* pl, unsigned site, C* row) {
+        const T2* q = IO::site(pl, site) + (size_t)r * NC * LINK_TILE;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) { T2 v = __ldg(q + c * LINK_TILE); row[c] = mk<T>(v.x, v.y); }
+    };
+    auto stage_row = [&](int buf, const C* row) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) M[buf][r * NC + c] = row[c];
+    };
+
+    C S[NC], A[NC], B[NC], D[NC], P[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) S[c] = mk<T>(0, 0);
+    const T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {
+        const int nu = k + (k >= mu ? 1 : 0);
+        const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+        const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+        const T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
+        const T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
+        // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+        load_row(pl_nu_s, cb, A);
+        load_row(pl_mu_o, cb + (unsigned)dpnu, B);
+        load_row(pl_nu_o, cb + (unsigned)dpmu, D);
+        stage_row(0, B);
+        stage_row(1, D);
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            C acc = mk<T>(0, 0);
+#pragma unroll
+            for (int q = 0; q < NC; ++q) mad(acc, A[q], M[0][q * NC + j]);
+            P[j] = acc;
+        }
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            C acc = S[j];
+#pragma unroll
+            for (int q = 0; q < NC; ++q) mad_cb(acc, P[q], M[1][j * NC + q]);
+            S[j] = acc;
+        }
+        // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
+        load_row(pl_nu_o, cb + (unsigned)dmnu, A);
+        load_row(pl_mu_o, cb + (unsigned)dmnu, B);
+        load_row(pl_nu_s, cb + (unsigned)(dmnu + dpmu), D);
+        stage_row(2, A);
+        stage_row(3, B);
+        stage_row(4, D);
+        __syncwarp();           // also orders the upper term's reads of buffers 0, 1 before their next writes
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            C acc = mk<T>(0, 0);
+#pragma unroll
+            for (int q = 0; q < NC; ++q) mad_ca(acc, M[2][q * NC + r], M[3][q * NC + j]);
+            P[j] = acc;
+        }
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            C acc = S[j];
+#pragma unroll
+            for (int q = 0; q < NC; ++q) mad(acc, P[q], M[4][q * NC + j]);
+            S[j] = acc;
+        }
+    }
+    // W = U S^dagger (step 2)
+    T2* pl_self = IO::plane(a.links, a.g, mu, p);
+    C U[NC], W[NC];
+    {
+        const T2* q = IO::site((const T2*)pl_self, cb) + (size_t)r * NC * LINK_TILE;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) { T2 v = __ldcs(q + c * LINK_TILE); U[c] = mk<T>(v.x, v.y); }
+    }
+    stage_row(0, S);            // buffer 0 was last read before the previous barrier
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < NC; ++j) {
+        C acc = mk<T>(0, 0);
+#pragma unroll
+        for (int q = 0; q < NC; ++q) mad_cb(acc, U[q], M[0][j * NC + q]);
+        W[j] = acc;
+    }
+
+    // steps 3-5: every SU(2) subgroup (i<j), lexicographic (reading R5)
+    const T beta = (T)a.beta;
+    const T two_beta_over_nc = (T)2 * beta / (T)NC;
+    const T m_nc_over_4beta = (T)-0.25 * (T)NC / beta;
+    const uint32_t c1 = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
+    const uint32_t c2_base = pack_c2(0, (int)a.pass, p, mu, 0);
+    unsigned att_total = 0, exhausted = 0;
+    int sub = 0;
+#pragma unroll 1
+    for (int i = 0; i < NC - 1; ++i) {
+#pragma unroll 1
+        for (int j = i + 1; j < NC; ++j, ++sub) {
+            const C wi = row_pick<NC, T>(W, i), wj = row_pick<NC, T>(W, j);
+            const C wii = shfl_cx(wi, gbase + i), wij = shfl_cx(wj, gbase + i);
+            const C wji = shfl_cx(wi, gbase + j), wjj = shfl_cx(wj, gbase + j);
+            T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
+            T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
+            const T n2 = r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3;
+            bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
+            T q4[4] = {(T)1, (T)0, (T)0, (T)0};
+            int used = 0;
+            if (ok) {
+                if (KIND == KIND_HB) {
+                    const T ik = Fn<T>::rsqrt(n2), kk = n2 * ik;
+                    T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
+                    T v[4];
+                    used = kp_draw<T>(two_beta_over_nc * kk, m_nc_over_4beta * ik, a.k0, a.k1, s.lex, c1,
+                                      c2_base | (uint32_t)sub, v);
+                    if (used) quat_mul(v, ud, q4); else ok = false;
+                } else {
+                    const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
+                    q4[0] = (r0 * r0 - (r1 * r1 + r2 * r2 + r3 * r3)) * in2;
+                    q4[1] = m2r0 * r1; q4[2] = m2r0 * r2; q4[3] = m2r0 * r3;
+                }
+            }
+            if (KIND == KIND_HB && owner && r == 0) {
+                att_total += (unsigned)used;
+                if (!ok) exhausted += 1u;
+                if (a.attempts) a.attempts[(size_t)sub * a.g.Vh + cb] = (uint8_t)(used > 255 ? 255 : used);
+            }
+            // rows i and j <- a . rows (eq 15): lane i needs row j and vice versa
+            const bool is_i = (r == i), is_j = (r == j);
+            const int partner = gbase + (is_i ? j : (is_j ? i : r));
+            // lane i: a00 own + a01 other ; lane j: a10 other + a11 own
+            const C c_own = is_i ? mk<T>(q4[0], q4[3]) : mk<T>(q4[0], -q4[3]);
+            const C c_oth = is_i ? mk<T>(q4[2], q4[1]) : mk<T>(-q4[2], q4[1]);
+            const bool rotate = ok && (is_i || is_j);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const C ou = shfl_cx(U[c], partner), ow = shfl_cx(W[c], partner);
+                if (rotate) {
+                    U[c] = is_i ? (c_own * U[c] + c_oth * ou) : (c_oth * ou + c_own * U[c]);
+                    W[c] = is_i ? (c_own * W[c] + c_oth * ow) : (c_oth * ow + c_own * W[c]);
+                }
+            }
+        }
+    }
+    if (owner) {
+        T2* q = IO::site(pl_self, cb) + (size_t)r * NC * LINK_TILE;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) __stcs(q + c * LINK_TILE, V2<T>::make(U[c].re, U[c].im));
+    }
+    if (KIND == KIND_HB) {
+        for (int o = 16; o > 0; o >>= 1) {
+            att_total += __shfl_down_sync(0xffffffffu, att_total, o);
+            exhausted += __shfl_down_sync(0xffffffffu, exhausted, o);
+        }
+        if (lane == 0) {
+            if (att_total) atomicAdd(a.counters, (unsigned long long)att_total);
+            if (exhausted) atomicAdd(a.counters + 1, (unsigned long long)exhausted);
+        }
+    }
+}
+
+template <int NC, class T>
+static cudaError_t launch_update_rows(int kind, const UpdateArgs& a, cudaStream_t st) {
+    constexpr int WARPS = RowsWarps<NC, T>::value;
+    const unsigned per_block = (unsigned)(WARPS * RowsCfg<NC>::LPW);
+    const unsigned grid = (a.g.Vh + per_block - 1) / per_block;
+    if (kind == KIND_HB) k_update_rows<NC, T, KIND_HB><<<grid, 32 * WARPS, 0, st>>>(a);
+    else                 k_update_rows<NC, T, KIND_OR><<<grid, 32 * WARPS, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace sug
