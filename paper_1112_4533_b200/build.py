@@ -18,7 +18,7 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
 ]
-HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", os.path.join("..", "..", "include", "su_gauge.h")]
+HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", "update_rows_kernel.cuh", os.path.join("..", "..", "include", "su_gauge.h")]
 
 
 def _units():

@@ -3,6 +3,7 @@
 // start, and the tiled-SoA <-> canonical-layout conversion used by export / import.
 // Compiled once per colour count with -DSUG_NC=<Nc>.
 #include "su_internal.h"
+#include "update_rows_kernel.cuh"
 
 #ifndef SUG_NC
 #error "compile with -DSUG_NC=<Nc>"
@@ -96,6 +97,118 @@ __global__ void __launch_bounds__(REDUCE_BLOCK) k_polyakov(const AuxArgs a) {
 #pragma unroll(UNR ? NC : 1)
         for (int d = 0; d < NC; ++d) { re += (double)P[d * NC + d].re; im += (double)P[d * NC + d].im; }
     }
+    re = block_sum(re);
+    im = block_sum(im);
+    if (threadIdx.x == 0) { a.partials[blockIdx.x] = re; a.partials[gridDim.x + blockIdx.x] = im; }
+}
+
+// ------------------------------------------------------------------------------------------
+// Row-per-lane forms of the two reductions for the generic SU(Nc) path (same decomposition as
+// update_rows_kernel.cuh): Nc lanes per site, lane r owns row r, the right-hand operands are
+// staged in shared memory (double-buffered: one __syncwarp per product pair).
+// ------------------------------------------------------------------------------------------
+template <int NC, class T>
+__global__ void __launch_bounds__(32 * RowsWarps<NC, T, 4>::value) k_plaquette_rows(const AuxArgs a) {
+    typedef RowsCfg<NC> Cfg;
+    typedef LinkIO<NC, T, STORE_FULL, true> IO;
+    typedef typename IO::T2 T2;
+    typedef cx<T> C;
+    constexpr int WARPS = RowsWarps<NC, T, 4>::value, LPW = Cfg::LPW, STRIDE = Cfg::STRIDE;
+    __shared__ C stage[WARPS * LPW][4][STRIDE];
+    const int lane = (int)(threadIdx.x & 31u), warp = (int)(threadIdx.x >> 5);
+    const bool shadow = lane >= LPW * NC;
+    const int g = shadow ? LPW - 1 : lane / NC;
+    const int r = shadow ? lane - LPW * NC : lane - g * NC;
+    const int p = (int)(blockIdx.x & 1u);
+    unsigned tix = ((blockIdx.x >> 1) * WARPS + (unsigned)warp) * LPW + (unsigned)g;
+    const bool owner = !shadow && tix < a.g.Vh;
+    if (tix >= a.g.Vh) tix = a.g.Vh - 1;
+    C(*M)[STRIDE] = stage[warp * LPW + g];
+    SiteNbr s;
+    site_of_thread(a.g, tix, p, s);
+    const unsigned cb = s.cb;
+    auto load_row = [&](int d, int par, unsigned site, C* row) {
+        const T2* q = IO::site(IO::plane((const void*)a.links, a.g, d, par), site) + (size_t)r * NC * LINK_TILE;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) { T2 v = __ldg(q + c * LINK_TILE); row[c] = mk<T>(v.x, v.y); }
+    };
+    C Uo[4][NC];
+#pragma unroll
+    for (int d = 0; d < 4; ++d) load_row(d, p, cb, Uo[d]);
+    double acc = 0.0;
+    int pair = 0;
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+        for (int nu = mu + 1; nu < 4; ++nu, ++pair) {
+            const int b0 = (pair & 1) * 2;
+            C B[NC], D[NC];
+            load_row(nu, 1 - p, cb + (unsigned)s.dp[mu], B);
+            load_row(mu, 1 - p, cb + (unsigned)s.dp[nu], D);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) { M[b0][r * NC + c] = B[c]; M[b0 + 1][r * NC + c] = D[c]; }
+            __syncwarp();
+            T t = 0;
+#pragma unroll
+            for (int j = 0; j < NC; ++j) {
+                C pj = mk<T>(0, 0), qj = mk<T>(0, 0);
+#pragma unroll
+                for (int q = 0; q < NC; ++q) { mad(pj, Uo[mu][q], M[b0][q * NC + j]); mad(qj, Uo[nu][q], M[b0 + 1][q * NC + j]); }
+                t += pj.re * qj.re + pj.im * qj.im;
+            }
+            if (owner) acc += (double)t;
+        }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) a.partials[blockIdx.x] = acc;
+}
+
+template <int NC, class T>
+__global__ void __launch_bounds__(32 * RowsWarps<NC, T, 2>::value) k_polyakov_rows(const AuxArgs a) {
+    typedef RowsCfg<NC> Cfg;
+    typedef LinkIO<NC, T, STORE_FULL, true> IO;
+    typedef typename IO::T2 T2;
+    typedef cx<T> C;
+    constexpr int WARPS = RowsWarps<NC, T, 2>::value, LPW = Cfg::LPW, STRIDE = Cfg::STRIDE;
+    __shared__ C stage[WARPS * LPW][2][STRIDE];
+    const int lane = (int)(threadIdx.x & 31u), warp = (int)(threadIdx.x >> 5);
+    const bool shadow = lane >= LPW * NC;
+    const int g = shadow ? LPW - 1 : lane / NC;
+    const int r = shadow ? lane - LPW * NC : lane - g * NC;
+    const unsigned Vs = (unsigned)a.g.L[0] * a.g.L[1] * a.g.L[2];
+    unsigned xs = (blockIdx.x * WARPS + (unsigned)warp) * LPW + (unsigned)g;
+    const bool owner = !shadow && xs < Vs;
+    if (xs >= Vs) xs = Vs - 1;
+    C(*M)[STRIDE] = stage[warp * LPW + g];
+    const int x = (int)(xs % (unsigned)a.g.L[0]);
+    const int y = (int)((xs / (unsigned)a.g.L[0]) % (unsigned)a.g.L[1]);
+    const int z = (int)(xs / ((unsigned)a.g.L[0] * a.g.L[1]));
+    auto load_row = [&](int t, C* row) {
+        const T2* q = IO::site(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), cb_of(a.g, x, y, z, t)) +
+                      (size_t)r * NC * LINK_TILE;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) { T2 v = __ldg(q + c * LINK_TILE); row[c] = mk<T>(v.x, v.y); }
+    };
+    C P[NC], A[NC], Q[NC];
+    load_row(0, P);
+#pragma unroll 1
+    for (int t = 1; t < a.g.L[3]; ++t) {
+        const int b = t & 1;
+        load_row(t, A);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) M[b][r * NC + c] = A[c];
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            C acc = mk<T>(0, 0);
+#pragma unroll
+            for (int q = 0; q < NC; ++q) mad(acc, P[q], M[b][q * NC + j]);
+            Q[j] = acc;
+        }
+#pragma unroll
+        for (int c = 0; c < NC; ++c) P[c] = Q[c];
+    }
+    const C d = row_pick<NC, T>(P, r);
+    double re = owner ? (double)d.re : 0.0, im = owner ? (double)d.im : 0.0;
     re = block_sum(re);
     im = block_sum(im);
     if (threadIdx.x == 0) { a.partials[blockIdx.x] = re; a.partials[gridDim.x + blockIdx.x] = im; }
@@ -381,8 +494,27 @@ __global__ void __launch_bounds__(128) k_import(const AuxArgs a) {
         ++*n_launch;                                                                                            \
     } while (0)
 
+// the generic path (and every Nc >= 5) measures with the row-per-lane kernels, except in the SU(2) quaternion /
+// SU(3) two-row layouts
+static bool use_rows(const Variant& v) { return SUG_NC >= 3 && v.store == STORE_FULL && (v.generic || SUG_NC > 4); }
+
 cudaError_t SUG_CAT(plaquette_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
-    const unsigned nb = plaquette_blocks(a.g.Vh);
+    unsigned nb = plaquette_blocks(a.g.Vh);
+#if SUG_NC >= 3
+    if (use_rows(v)) {
+        constexpr int NC = SUG_NC;
+        if (v.prec == SU_FP64) {
+            constexpr unsigned PB = RowsWarps<NC, double, 4>::value * RowsCfg<NC>::LPW;
+            nb = 2u * ((a.g.Vh + PB - 1) / PB);
+            k_plaquette_rows<NC, double><<<nb, 32 * RowsWarps<NC, double, 4>::value, 0, st>>>(a);
+        } else {
+            constexpr unsigned PB = RowsWarps<NC, float, 4>::value * RowsCfg<NC>::LPW;
+            nb = 2u * ((a.g.Vh + PB - 1) / PB);
+            k_plaquette_rows<NC, float><<<nb, 32 * RowsWarps<NC, float, 4>::value, 0, st>>>(a);
+        }
+        ++*n_launch;
+    } else
+#endif
     SUG_MEAS_DISPATCH(k_plaquette, nb, PLAQ_BLOCK);
     const double scale = 1.0 / (6.0 * 2.0 * (double)a.g.Vh * (double)SUG_NC);
     k_reduce_final<<<1, REDUCE_BLOCK, 0, st>>>(a.partials, nb, 1, scale, a.result);
@@ -392,7 +524,22 @@ cudaError_t SUG_CAT(plaquette_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cu
 
 cudaError_t SUG_CAT(polyakov_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
     const unsigned Vs = (unsigned)a.g.L[0] * a.g.L[1] * a.g.L[2];
-    const unsigned nb = reduce_blocks(Vs);
+    unsigned nb = reduce_blocks(Vs);
+#if SUG_NC >= 3
+    if (use_rows(v)) {
+        constexpr int NC = SUG_NC;
+        if (v.prec == SU_FP64) {
+            constexpr unsigned PB = RowsWarps<NC, double, 2>::value * RowsCfg<NC>::LPW;
+            nb = (Vs + PB - 1) / PB;
+            k_polyakov_rows<NC, double><<<nb, 32 * RowsWarps<NC, double, 2>::value, 0, st>>>(a);
+        } else {
+            constexpr unsigned PB = RowsWarps<NC, float, 2>::value * RowsCfg<NC>::LPW;
+            nb = (Vs + PB - 1) / PB;
+            k_polyakov_rows<NC, float><<<nb, 32 * RowsWarps<NC, float, 2>::value, 0, st>>>(a);
+        }
+        ++*n_launch;
+    } else
+#endif
     SUG_MEAS_DISPATCH(k_polyakov, nb, REDUCE_BLOCK);
     k_reduce_final<<<1, REDUCE_BLOCK, 0, st>>>(a.partials, nb, 2, 1.0 / ((double)Vs * (double)SUG_NC), a.result);
     ++*n_launch;

@@ -264,7 +264,9 @@ su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precis
         h->owns_links = (st == SU_OK);
     }
     const unsigned Vs = (unsigned)Lx * Ly * Lz;
-    const size_t npart = (size_t)plaquette_blocks(h->g.Vh) + 2 * (size_t)reduce_blocks(Vs) + 2;
+    // partial sums of the reductions: one per block; the row-per-lane kernels have as few as 4 sites per block
+    const size_t npart = (h->var.generic ? 2 * ((size_t)h->g.Vh / ROWS_MIN_LINKS_PER_BLOCK + 1)
+                                         : (size_t)plaquette_blocks(h->g.Vh) + 2 * (size_t)reduce_blocks(Vs)) + 2;
     if (st == SU_OK && cudaMalloc(&h->d_partials, npart * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_result, 2 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_counters, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ENOMEM;

@@ -47,6 +47,7 @@ SUG_DECLARE_NC(8)
 
 constexpr int REDUCE_BLOCK = 256;
 inline unsigned reduce_blocks(unsigned n) { return (n + REDUCE_BLOCK - 1) / REDUCE_BLOCK; }
+constexpr int ROWS_MIN_LINKS_PER_BLOCK = 4;   // row-per-lane kernels: 1 warp x floor(32 / SU_MAX_NC) sites per block at least
 constexpr int PLAQ_BLOCK = 128;          // plaquette kernel: blocks alternate parity over the same region
 #ifndef PLAQ_MINB
 #define PLAQ_MINB 3

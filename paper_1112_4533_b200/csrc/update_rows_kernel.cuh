@@ -21,12 +21,12 @@ template <int NC> struct RowsCfg {
     static constexpr int LPW = 32 / NC;                       // links per warp
     static constexpr int STRIDE = NC * NC + 1;                // complex elements per staged matrix (+1: bank spread)
     static constexpr int NBUF = 5;                            // upper term: B, C; lower term: A, B, C
-    static constexpr size_t bytes(int w, size_t real) { return (size_t)w * LPW * NBUF * STRIDE * 2 * real; }
+    static constexpr size_t bytes(int w, size_t real, int nbuf) { return (size_t)w * LPW * nbuf * STRIDE * 2 * real; }
 };
-// warps per block: as many (<= 4) as keep the staging area within 48 KB of static shared memory
-template <int NC, class T> struct RowsWarps {
+// warps per block: as many (<= 4) as keep NB staged matrices per link within 48 KB of static shared memory
+template <int NC, class T, int NB = RowsCfg<NC>::NBUF> struct RowsWarps {
     static constexpr size_t LIM = 48 * 1024, R = sizeof(T);
-    static constexpr int value = RowsCfg<NC>::bytes(4, R) <= LIM ? 4 : (RowsCfg<NC>::bytes(3, R) <= LIM ? 3 : (RowsCfg<NC>::bytes(2, R) <= LIM ? 2 : 1));
+    static constexpr int value = RowsCfg<NC>::bytes(4, R, NB) <= LIM ? 4 : (RowsCfg<NC>::bytes(3, R, NB) <= LIM ? 3 : (RowsCfg<NC>::bytes(2, R, NB) <= LIM ? 2 : 1));
 };
 
 template <class T> __device__ __forceinline__ cx<T> shfl_cx(cx<T> v, int src) {

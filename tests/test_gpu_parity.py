@@ -26,9 +26,10 @@ VARIANTS = [
     (3, "fp64", False, "auto"), (3, "fp32", False, "auto"), (3, "fp64", True, "auto"), (3, "fp32", True, "auto"),
     (3, "fp64", False, "generic"), (3, "fp32", True, "generic"),
     (4, "fp64", False, "auto"), (4, "fp32", False, "auto"), (4, "fp64", False, "generic"), (4, "fp32", False, "generic"),
-    (5, "fp64", False, "auto"), (6, "fp64", False, "auto"), (6, "fp32", False, "auto"), (8, "fp64", False, "auto"),
+    (5, "fp64", False, "auto"), (6, "fp64", False, "auto"), (6, "fp32", False, "auto"), (7, "fp64", False, "auto"),
+    (8, "fp64", False, "auto"),
 ]
-BETA = {2: 2.3, 3: 6.0, 4: 11.0, 5: 17.0, 6: 25.0, 8: 44.0}
+BETA = {2: 2.3, 3: 6.0, 4: 11.0, 5: 17.0, 6: 25.0, 7: 34.0, 8: 44.0}
 
 
 def _ids(v):
