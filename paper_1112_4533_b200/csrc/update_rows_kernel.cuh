@@ -7,9 +7,10 @@
 //   staple term  S_r += (A_r . B) . C^dagger         A_r in registers, B and C staged in shared memory
 //                S_r += (A^dagger B)_r . C           A, B, C staged in shared memory
 //   W_r = U_r . S^dagger                             S staged in shared memory
-//   subgroup (i,j): lanes i and j exchange rows by warp shuffle, every lane of the group evaluates
-//                   the 2x2 projection and the Kennedy-Pendleton draw redundantly (no extra cost in
-//                   SIMT: the lanes would idle otherwise), rows i and j are rotated (eq 15).
+//   subgroup (i,j): lanes i and j exchange the four entries of the 2x2 block and their rows by warp
+//                   shuffle, both evaluate the projection and the Kennedy-Pendleton draw (same counter
+//                   -> same numbers) and rotate their own row (eq 15); subgroups on disjoint row pairs
+//                   commute exactly, so the lexicographic sequence runs as a wavefront of 2 Nc - 3 slots.
 // A warp holds floor(32 / Nc) links; left-over lanes shadow the last group and never store.
 // The order of operations inside every sum is the one of update_kernel.cuh and of the oracle.
 #pragma once
@@ -157,53 +158,56 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value) k_update_rows(co
     const uint32_t c1 = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
     const uint32_t c2_base = pack_c2(0, (int)a.pass, p, mu, 0);
     unsigned att_total = 0, exhausted = 0;
-    int sub = 0;
+    // Wavefront over the lexicographic subgroup order: step (i,j) only depends on earlier steps that touched
+    // row i or row j, and steps on disjoint row pairs commute exactly (A_ij is built from rows i,j of W and
+    // rotates rows i,j only). All pairs with i + j = t + 1 are disjoint and have all their predecessors in
+    // earlier slots, so slot t runs them at once: 2 Nc - 3 slots instead of Nc (Nc - 1) / 2 steps, every lane
+    // busy in most of them, with the result of the sequential order (the reordered steps commute exactly).
 #pragma unroll 1
-    for (int i = 0; i < NC - 1; ++i) {
-#pragma unroll 1
-        for (int j = i + 1; j < NC; ++j, ++sub) {
-            const C wi = row_pick<NC, T>(W, i), wj = row_pick<NC, T>(W, j);
-            const C wii = shfl_cx(wi, gbase + i), wij = shfl_cx(wj, gbase + i);
-            const C wji = shfl_cx(wi, gbase + j), wjj = shfl_cx(wj, gbase + j);
-            T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
-            T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
-            const T n2 = r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3;
-            bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
-            T q4[4] = {(T)1, (T)0, (T)0, (T)0};
-            int used = 0;
-            if (ok) {
-                if (KIND == KIND_HB) {
-                    const T ik = Fn<T>::rsqrt(n2), kk = n2 * ik;
-                    T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
-                    T v[4];
-                    used = kp_draw<T>(two_beta_over_nc * kk, m_nc_over_4beta * ik, a.k0, a.k1, s.lex, c1,
-                                      c2_base | (uint32_t)sub, v);
-                    if (used) quat_mul(v, ud, q4); else ok = false;
-                } else {
-                    const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
-                    q4[0] = (r0 * r0 - (r1 * r1 + r2 * r2 + r3 * r3)) * in2;
-                    q4[1] = m2r0 * r1; q4[2] = m2r0 * r2; q4[3] = m2r0 * r3;
-                }
+    for (int t = 0; t <= 2 * NC - 4; ++t) {
+        const int sidx = t + 1 - r;
+        const bool paired = sidx >= 0 && sidx < NC && sidx != r;
+        const int pr = paired ? sidx : r;                       // partner row (self when idle in this slot)
+        const bool is_i = r < pr;
+        const int i = is_i ? r : pr, j = is_i ? pr : r;
+        const int sub = i * NC - (i * (i + 1)) / 2 + (j - i - 1);   // lexicographic index of (i,j)
+        const C wd = row_pick<NC, T>(W, r), wo = row_pick<NC, T>(W, pr);       // W_rr, W_r,pr
+        const C pd = shfl_cx(wd, gbase + pr), po = shfl_cx(wo, gbase + pr);     // W_pr,pr, W_pr,r
+        const C wii = is_i ? wd : pd, wij = is_i ? wo : po, wji = is_i ? po : wo, wjj = is_i ? pd : wd;
+        T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
+        T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
+        const T n2 = r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3;
+        bool ok = paired && (n2 > (T)0) && Fn<T>::finite(n2);
+        T q4[4] = {(T)1, (T)0, (T)0, (T)0};
+        int used = 0;
+        if (ok) {
+            if (KIND == KIND_HB) {
+                const T ik = Fn<T>::rsqrt(n2), kk = n2 * ik;
+                T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
+                T v[4];
+                used = kp_draw<T>(two_beta_over_nc * kk, m_nc_over_4beta * ik, a.k0, a.k1, s.lex, c1,
+                                  c2_base | (uint32_t)sub, v);
+                if (used) quat_mul(v, ud, q4); else ok = false;
+            } else {
+                const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
+                q4[0] = (r0 * r0 - (r1 * r1 + r2 * r2 + r3 * r3)) * in2;
+                q4[1] = m2r0 * r1; q4[2] = m2r0 * r2; q4[3] = m2r0 * r3;
             }
-            if (KIND == KIND_HB && owner && r == 0) {
-                att_total += (unsigned)used;
-                if (!ok) exhausted += 1u;
-                if (a.attempts) a.attempts[(size_t)sub * a.g.Vh + cb] = (uint8_t)(used > 255 ? 255 : used);
-            }
-            // rows i and j <- a . rows (eq 15): lane i needs row j and vice versa
-            const bool is_i = (r == i), is_j = (r == j);
-            const int partner = gbase + (is_i ? j : (is_j ? i : r));
-            // lane i: a00 own + a01 other ; lane j: a10 other + a11 own
-            const C c_own = is_i ? mk<T>(q4[0], q4[3]) : mk<T>(q4[0], -q4[3]);
-            const C c_oth = is_i ? mk<T>(q4[2], q4[1]) : mk<T>(-q4[2], q4[1]);
-            const bool rotate = ok && (is_i || is_j);
+        }
+        if (KIND == KIND_HB && owner && paired && is_i) {        // lane i of the pair keeps the books
+            att_total += (unsigned)used;
+            if (!ok) exhausted += 1u;
+            if (a.attempts) a.attempts[(size_t)sub * a.g.Vh + cb] = (uint8_t)(used > 255 ? 255 : used);
+        }
+        // rows i and j <- a . rows (eq 15): lane i: a00 own + a01 other ; lane j: a10 other + a11 own
+        const C c_own = is_i ? mk<T>(q4[0], q4[3]) : mk<T>(q4[0], -q4[3]);
+        const C c_oth = is_i ? mk<T>(q4[2], q4[1]) : mk<T>(-q4[2], q4[1]);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                const C ou = shfl_cx(U[c], partner), ow = shfl_cx(W[c], partner);
-                if (rotate) {
-                    U[c] = is_i ? (c_own * U[c] + c_oth * ou) : (c_oth * ou + c_own * U[c]);
-                    W[c] = is_i ? (c_own * W[c] + c_oth * ow) : (c_oth * ow + c_own * W[c]);
-                }
+        for (int c = 0; c < NC; ++c) {
+            const C ou = shfl_cx(U[c], gbase + pr), ow = shfl_cx(W[c], gbase + pr);
+            if (ok) {
+                U[c] = is_i ? (c_own * U[c] + c_oth * ou) : (c_oth * ou + c_own * U[c]);
+                W[c] = is_i ? (c_own * W[c] + c_oth * ow) : (c_oth * ow + c_own * W[c]);
             }
         }
     }
