@@ -126,6 +126,37 @@ su_status su_get_timing(su_lattice*, double* hb_ms, uint64_t* hb_launches, doubl
 /* Number of kernels this handle has launched so far (for the benchmark's gpu_launches). */
 su_status su_get_launch_count(su_lattice*, uint64_t* out);
 
+/* ---- t-slab decomposition over several GPUs (Fig. 2: "each GPU holds Lt/n + 2 slices") ----
+ * A slab handle owns the global time slices [t0, t0 + Lt_local) of an Lx x Ly x Lz x Lt_global lattice and
+ * stores one halo slice below and one above them. Lt_local even and >= 2, the same on every slab;
+ * Lx Ly Lz / 2 a multiple of 32 (else SU_EUNSUPPORTED). The Philox site index is the GLOBAL one, so n slabs
+ * reproduce the single-lattice chain exactly.
+ *   - su_slab_set_peers: DEVICE pointers (valid on this handle's device: same process, peer access, or
+ *     su_ipc_open) to the link buffers of the slabs below (t0 - Lt_local) and above (t0 + Lt_local),
+ *     periodically; a lattice cut into one slab names itself twice. The update kernel stores every link of
+ *     the first / last owned slice into that neighbour's halo as well (fused halo push: no separate exchange).
+ *   - Ordering is the caller's: sub-step k+1 may start on any slab only after sub-step k has finished on
+ *     its neighbours (stream order in one process; a stream-ordered collective or event across processes).
+ *     su_sweep therefore returns SU_ESTATE on one slab of several; drive su_substep. Sub-step (p, mu) never
+ *     reads the halo plane (mu, p), which is the only one its neighbours write meanwhile.
+ *   - su_init_cold / su_init_hot / su_reunitarize fill or transform the halos consistently by themselves;
+ *     after su_import_links every slab must call su_slab_halo_push once all slabs have imported.
+ *   - su_plaquette returns this slab's SHARE (sum over slabs = the plaquette); su_polyakov and the
+ *     attempt-count output of su_substep are SU_EUNSUPPORTED; import / export move the owned slices,
+ *     n_doubles = 4 * Lx Ly Lz Lt_local * 2 Nc^2.
+ *   - su_slab_bytes: size of the link buffer (0 on invalid arguments). su_slab_links: its device address.
+ *   - su_ipc_export / su_ipc_open / su_ipc_close: CUDA IPC handle (64 bytes) of a library-owned link buffer,
+ *     for peers in other processes. */
+su_status su_lattice_create_slab(int Nc, int Lx, int Ly, int Lz, int Lt_global, int t0, int Lt_local,
+                                 su_precision p, const su_options* opt, su_lattice** out);
+size_t    su_slab_bytes(int Nc, int Lx, int Ly, int Lz, int Lt_local, su_precision p, su_storage s);
+su_status su_slab_links(su_lattice*, void** device_links, size_t* bytes);
+su_status su_slab_set_peers(su_lattice*, void* device_links_below, void* device_links_above);
+su_status su_slab_halo_push(su_lattice*);
+su_status su_ipc_export(su_lattice*, unsigned char handle[64]);
+su_status su_ipc_open(su_lattice*, const unsigned char handle[64], void** device_ptr);
+su_status su_ipc_close(su_lattice*, void* device_ptr);
+
 /* Text of the last error on this handle ("" if none); static text if the handle is NULL.
  * Owned by the library, valid until the next call on the handle. */
 const char* su_last_error(const su_lattice*);

@@ -29,6 +29,8 @@ ABI_SYMBOLS = (
     "su_init_cold", "su_init_hot", "su_sweep", "su_plaquette", "su_polyakov", "su_reunitarize",
     "su_export_links", "su_import_links", "su_set_rng", "su_substep", "su_get_counters",
     "su_synchronize", "su_set_graph_mode", "su_set_timing", "su_get_timing", "su_get_launch_count", "su_last_error",
+    "su_lattice_create_slab", "su_slab_bytes", "su_slab_links", "su_slab_set_peers", "su_slab_halo_push",
+    "su_ipc_export", "su_ipc_open", "su_ipc_close",
 )
 
 
@@ -79,8 +81,17 @@ def lib():
     L.su_get_launch_count.argtypes = [P, C.POINTER(C.c_uint64)]
     L.su_last_error.argtypes = [P]
     L.su_last_error.restype = C.c_char_p
+    L.su_lattice_create_slab.argtypes = [I] * 8 + [C.POINTER(su_options), C.POINTER(P)]
+    L.su_slab_bytes.argtypes = [I] * 7
+    L.su_slab_bytes.restype = C.c_size_t
+    L.su_slab_links.argtypes = [P, C.POINTER(P), C.POINTER(C.c_size_t)]
+    L.su_slab_set_peers.argtypes = [P, P, P]
+    L.su_slab_halo_push.argtypes = [P]
+    L.su_ipc_export.argtypes = [P, C.c_char_p]
+    L.su_ipc_open.argtypes = [P, C.c_char_p, C.POINTER(P)]
+    L.su_ipc_close.argtypes = [P, P]
     for name in ABI_SYMBOLS:
-        if name not in ("su_lattice_bytes", "su_last_error"):
+        if name not in ("su_lattice_bytes", "su_slab_bytes", "su_last_error"):
             getattr(L, name).restype = I
     _lib = L
     return L
@@ -105,7 +116,11 @@ class Lattice:
     uint8 tensor on `device`, kernels run on torch's current stream at construction time.
     """
 
-    def __init__(self, Nc, dims, precision="fp64", recon12=False, kernel="auto", device=0, graph=False):
+    def __init__(self, Nc, dims, precision="fp64", recon12=False, kernel="auto", device=0, graph=False, slab=None,
+                 library_buffer=False):
+        """slab = (t0, Lt_local): this handle owns the global time slices [t0, t0 + Lt_local) of the lattice
+        `dims` (su_lattice_create_slab); see SlabGroup / DistributedLattice in .slab for the drivers.
+        library_buffer: let the library cudaMalloc the links (needed for CUDA IPC) instead of a torch tensor."""
         import torch
 
         if not torch.cuda.is_available():
@@ -114,24 +129,35 @@ class Lattice:
         self.Nc, self.dims = int(Nc), tuple(int(d) for d in dims)
         self.precision = "fp64" if _prec(precision) == SU_FP64 else "fp32"
         self.recon12 = bool(recon12)
-        self.V = int(np.prod(self.dims))
+        self.slab = None if slab is None else (int(slab[0]), int(slab[1]))
+        self.local_dims = self.dims if slab is None else self.dims[:3] + (self.slab[1],)
+        self.V = int(np.prod(self.local_dims))              # owned sites
         self.n_sub = self.Nc * (self.Nc - 1) // 2
         self._h = C.c_void_p()
         self._torch = torch
         self.device = torch.device("cuda", device) if isinstance(device, int) else torch.device(device)
         storage = SU_STORE_RECON12 if recon12 else SU_STORE_FULL
-        nbytes = L.su_lattice_bytes(self.Nc, *self.dims, _prec(precision), storage)
+        if slab is None:
+            nbytes = L.su_lattice_bytes(self.Nc, *self.dims, _prec(precision), storage)
+        else:
+            nbytes = L.su_slab_bytes(self.Nc, *self.dims[:3], self.slab[1], _prec(precision), storage)
         if nbytes == 0:
             raise SuError(SU_EINVAL, "su_lattice_bytes", "invalid Nc / extents / storage")
         with torch.cuda.device(self.device):
-            self.buffer = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.buffer = None if library_buffer else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = torch.cuda.current_stream(self.device)
         opt = su_options(storage, {"auto": 0, "specialised": 1, "generic": 2}[kernel], self.device.index or 0,
-                         C.c_void_p(self.stream.cuda_stream), C.c_void_p(self.buffer.data_ptr()), nbytes)
-        st = L.su_lattice_create_ex(self.Nc, *self.dims, _prec(precision), C.byref(opt), C.byref(self._h))
+                         C.c_void_p(self.stream.cuda_stream),
+                         C.c_void_p(self.buffer.data_ptr()) if self.buffer is not None else None,
+                         nbytes if self.buffer is not None else 0)
+        if slab is None:
+            st = L.su_lattice_create_ex(self.Nc, *self.dims, _prec(precision), C.byref(opt), C.byref(self._h))
+        else:
+            st = L.su_lattice_create_slab(self.Nc, *self.dims, self.slab[0], self.slab[1], _prec(precision),
+                                          C.byref(opt), C.byref(self._h))
         if st != SU_OK:
             self._h = C.c_void_p()
-            raise SuError(st, "su_lattice_create_ex")
+            raise SuError(st, "su_lattice_create_slab" if slab else "su_lattice_create_ex")
         if graph:
             self.set_graph_mode(True)
 
@@ -192,7 +218,7 @@ class Lattice:
 
     def export_links(self, out=None):
         """-> complex128 array [t][z][y][x][mu][row][col] (host)"""
-        Lx, Ly, Lz, Lt = self.dims
+        Lx, Ly, Lz, Lt = self.local_dims
         if out is None:
             out = np.empty((Lt, Lz, Ly, Lx, 4, self.Nc, self.Nc), dtype=np.complex128)
         self._ck(lib().su_export_links(self._h, out.ctypes.data, out.size * 2), "su_export_links")
@@ -222,6 +248,31 @@ class Lattice:
         na, nb = C.c_uint64(), C.c_uint64()
         self._ck(lib().su_get_timing(self._h, C.byref(a), C.byref(na), C.byref(b), C.byref(nb)), "su_get_timing")
         return {"hb_ms": a.value, "hb_launches": na.value, "or_ms": b.value, "or_launches": nb.value}
+
+    # ---- t-slab decomposition (include/su_gauge.h "t-slab decomposition") ----
+    def links_ptr(self):
+        p, n = C.c_void_p(), C.c_size_t()
+        self._ck(lib().su_slab_links(self._h, C.byref(p), C.byref(n)), "su_slab_links")
+        return p.value, n.value
+
+    def set_peers(self, below_ptr, above_ptr):
+        self._ck(lib().su_slab_set_peers(self._h, C.c_void_p(below_ptr), C.c_void_p(above_ptr)), "su_slab_set_peers")
+
+    def halo_push(self):
+        self._ck(lib().su_slab_halo_push(self._h), "su_slab_halo_push")
+
+    def ipc_export(self):
+        buf = C.create_string_buffer(64)
+        self._ck(lib().su_ipc_export(self._h, buf), "su_ipc_export")
+        return buf.raw
+
+    def ipc_open(self, handle):
+        p = C.c_void_p()
+        self._ck(lib().su_ipc_open(self._h, C.create_string_buffer(handle, 64), C.byref(p)), "su_ipc_open")
+        return p.value
+
+    def ipc_close(self, ptr):
+        self._ck(lib().su_ipc_close(self._h, C.c_void_p(ptr)), "su_ipc_close")
 
     def launch_count(self):
         n = C.c_uint64()

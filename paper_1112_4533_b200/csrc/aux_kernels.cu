@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(PLAQ_BLOCK, PLAQ_MINB) k_plaquette(const AuxAr
     const int p = (int)(blockIdx.x & 1u);
     const unsigned tix = (blockIdx.x >> 1) * PLAQ_BLOCK + threadIdx.x;
     double acc = 0.0;
-    if (tix < a.g.Vh) {
+    if (tix < a.g.Vh_int) {
         SiteNbr s;
         site_of_thread(a.g, tix, p, s);
         const unsigned cb = s.cb;
@@ -86,10 +86,10 @@ __global__ void __launch_bounds__(REDUCE_BLOCK) k_polyakov(const AuxArgs a) {
         const int y = (int)((xs / (unsigned)a.g.L[0]) % (unsigned)a.g.L[1]);
         const int z = (int)(xs / ((unsigned)a.g.L[0] * a.g.L[1]));
         C P[NC * NC], A[NC * NC], Q[NC * NC];
-        IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z) & 1), cb_of(a.g, x, y, z, 0), P);
+        IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, site_parity(a.g, x, y, z, 0)), cb_of(a.g, x, y, z, 0), P);
 #pragma unroll 1
         for (int t = 1; t < a.g.L[3]; ++t) {
-            IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), cb_of(a.g, x, y, z, t), A);
+            IO::template load<LD_RO>(IO::plane((const void*)a.links, a.g, 3, site_parity(a.g, x, y, z, t)), cb_of(a.g, x, y, z, t), A);
             M::mul_nn(P, A, Q);
 #pragma unroll(UNR ? NC * NC : 1)
             for (int e = 0; e < NC * NC; ++e) P[e] = Q[e];
@@ -121,8 +121,8 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T, 4>::value) k_plaquette_r
     const int r = shadow ? lane - LPW * NC : lane - g * NC;
     const int p = (int)(blockIdx.x & 1u);
     unsigned tix = ((blockIdx.x >> 1) * WARPS + (unsigned)warp) * LPW + (unsigned)g;
-    const bool owner = !shadow && tix < a.g.Vh;
-    if (tix >= a.g.Vh) tix = a.g.Vh - 1;
+    const bool owner = !shadow && tix < a.g.Vh_int;
+    if (tix >= a.g.Vh_int) tix = a.g.Vh_int - 1;
     C(*M)[STRIDE] = stage[warp * LPW + g];
     SiteNbr s;
     site_of_thread(a.g, tix, p, s);
@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T, 2>::value) k_polyakov_ro
     const int y = (int)((xs / (unsigned)a.g.L[0]) % (unsigned)a.g.L[1]);
     const int z = (int)(xs / ((unsigned)a.g.L[0] * a.g.L[1]));
     auto load_row = [&](int t, C* row) {
-        const T2* q = IO::site(IO::plane((const void*)a.links, a.g, 3, (x + y + z + t) & 1), cb_of(a.g, x, y, z, t)) +
+        const T2* q = IO::site(IO::plane((const void*)a.links, a.g, 3, site_parity(a.g, x, y, z, t)), cb_of(a.g, x, y, z, t)) +
                       (size_t)r * NC * LINK_TILE;
 #pragma unroll
         for (int c = 0; c < NC; ++c) { T2 v = __ldg(q + c * LINK_TILE); row[c] = mk<T>(v.x, v.y); }
@@ -428,10 +428,10 @@ __global__ void __launch_bounds__(128) k_export(const AuxArgs a) {
     unsigned r = s / (unsigned)a.g.L[0];
     const int y = (int)(r % (unsigned)a.g.L[1]); r /= (unsigned)a.g.L[1];
     const int z = (int)(r % (unsigned)a.g.L[2]);
-    const int t = (int)(r / (unsigned)a.g.L[2]);
-    const int p = (x + y + z + t) & 1;
+    const int t = (int)(r / (unsigned)a.g.L[2]) + a.g.t_halo;                // stored slice of owned slice t
+    const int p = site_parity(a.g, x, y, z, t);
     cx<T> U[NC * NC];
-    IO::template load<LD_PLAIN>(IO::plane((const void*)a.links, a.g, mu, p), s >> 1, U);
+    IO::template load<LD_PLAIN>(IO::plane((const void*)a.links, a.g, mu, p), cb_of(a.g, x, y, z, t), U);
     double2* dst = (double2*)a.staging + (size_t)l * NC * NC;
     for (int e = 0; e < NC * NC; ++e) dst[e] = make_double2((double)U[e].re, (double)U[e].im);
 }
@@ -447,12 +447,12 @@ __global__ void __launch_bounds__(128) k_import(const AuxArgs a) {
     unsigned r = s / (unsigned)a.g.L[0];
     const int y = (int)(r % (unsigned)a.g.L[1]); r /= (unsigned)a.g.L[1];
     const int z = (int)(r % (unsigned)a.g.L[2]);
-    const int t = (int)(r / (unsigned)a.g.L[2]);
-    const int p = (x + y + z + t) & 1;
+    const int t = (int)(r / (unsigned)a.g.L[2]) + a.g.t_halo;
+    const int p = site_parity(a.g, x, y, z, t);
     const double2* src = (const double2*)a.staging + (size_t)l * NC * NC;
     cx<T> U[NC * NC];
     for (int e = 0; e < NC * NC; ++e) { double2 v = src[e]; U[e] = mk<T>((T)v.x, (T)v.y); }
-    IO::store(IO::plane(a.links, a.g, mu, p), s >> 1, U);
+    IO::store(IO::plane(a.links, a.g, mu, p), cb_of(a.g, x, y, z, t), U);
 }
 
 // ---- dispatch -----------------------------------------------------------------------------
@@ -499,24 +499,25 @@ __global__ void __launch_bounds__(128) k_import(const AuxArgs a) {
 static bool use_rows(const Variant& v) { return SUG_NC >= 3 && v.store == STORE_FULL && (v.generic || SUG_NC > 4); }
 
 cudaError_t SUG_CAT(plaquette_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
-    unsigned nb = plaquette_blocks(a.g.Vh);
+    unsigned nb = plaquette_blocks(a.g.Vh_int);
 #if SUG_NC >= 3
     if (use_rows(v)) {
         constexpr int NC = SUG_NC;
         if (v.prec == SU_FP64) {
             constexpr unsigned PB = RowsWarps<NC, double, 4>::value * RowsCfg<NC>::LPW;
-            nb = 2u * ((a.g.Vh + PB - 1) / PB);
+            nb = 2u * ((a.g.Vh_int + PB - 1) / PB);
             k_plaquette_rows<NC, double><<<nb, 32 * RowsWarps<NC, double, 4>::value, 0, st>>>(a);
         } else {
             constexpr unsigned PB = RowsWarps<NC, float, 4>::value * RowsCfg<NC>::LPW;
-            nb = 2u * ((a.g.Vh + PB - 1) / PB);
+            nb = 2u * ((a.g.Vh_int + PB - 1) / PB);
             k_plaquette_rows<NC, float><<<nb, 32 * RowsWarps<NC, float, 4>::value, 0, st>>>(a);
         }
         ++*n_launch;
     } else
 #endif
     SUG_MEAS_DISPATCH(k_plaquette, nb, PLAQ_BLOCK);
-    const double scale = 1.0 / (6.0 * 2.0 * (double)a.g.Vh * (double)SUG_NC);
+    // normalised by the GLOBAL volume: in slab mode the result is this slab's share of the plaquette
+    const double scale = 1.0 / (6.0 * 2.0 * (double)a.g.Vsh * (double)a.g.Lt_glob * (double)SUG_NC);
     k_reduce_final<<<1, REDUCE_BLOCK, 0, st>>>(a.partials, nb, 1, scale, a.result);
     ++*n_launch;
     return cudaGetLastError();

@@ -23,6 +23,8 @@ struct su_lattice {
     int device = 0;
     cudaStream_t stream = nullptr;
     void* links = nullptr;
+    void* peer_lo = nullptr;       // slab mode: link buffers of the slabs below / above (su_slab_set_peers)
+    void* peer_hi = nullptr;
     bool owns_links = false;
     size_t links_bytes = 0;
     double* d_partials = nullptr;
@@ -138,6 +140,8 @@ su_status launch_substep(su_lattice* h, double beta, int kind, int pass, int par
     a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
     a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = (uint32_t)pass;
     a.attempts = d_attempts; a.counters = h->d_counters;
+    a.peer_lo = h->peer_lo; a.peer_hi = h->peer_hi;
+    if (h->g.t_halo && (!h->peer_lo || !h->peer_hi)) return fail(h, SU_ESTATE, "slab lattice: su_slab_set_peers first");
     SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "update kernel launch");
     return SU_OK;
 }
@@ -221,28 +225,42 @@ su_status su_lattice_create(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision
     return su_lattice_create_ex(Nc, Lx, Ly, Lz, Lt, p, nullptr, out);
 }
 
-su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, const su_options* opt,
-                               su_lattice** out) {
+// Lt_glob / t0 / Lt_loc: the handle owns global time slices [t0, t0 + Lt_loc); slab = false: the whole lattice.
+static su_status create_common(int Nc, int Lx, int Ly, int Lz, int Lt_glob, bool slab, int t0, int Lt_loc, su_precision p,
+                               const su_options* opt, su_lattice** out) {
     if (!out) return SU_EINVAL;
     su_options o{};
     o.storage = SU_STORE_FULL; o.kernel = SU_KERNEL_AUTO; o.device = -1;
     if (opt) o = *opt;
-    if (!dims_ok(Nc, Lx, Ly, Lz, Lt)) return SU_EINVAL;
+    if (!dims_ok(Nc, Lx, Ly, Lz, Lt_glob)) return SU_EINVAL;
     if (p != SU_FP32 && p != SU_FP64) return SU_EINVAL;
     if (o.storage != SU_STORE_FULL && o.storage != SU_STORE_RECON12) return SU_EINVAL;
     if (o.storage == SU_STORE_RECON12 && Nc != 3) return SU_EINVAL;
     if (o.kernel != SU_KERNEL_AUTO && o.kernel != SU_KERNEL_SPECIALISED && o.kernel != SU_KERNEL_GENERIC) return SU_EINVAL;
     if (Nc > SU_MAX_NC) return SU_EUNSUPPORTED;
     if (o.kernel == SU_KERNEL_SPECIALISED && Nc > 4) return SU_EUNSUPPORTED;
+    if (slab) {
+        // whole 32-site tiles per time slice and parity, so that a halo slice of a plane is one contiguous range
+        if (Lt_loc < 2 || (Lt_loc & 1) || t0 < 0 || t0 + Lt_loc > Lt_glob) return SU_EINVAL;
+        if (((size_t)Lx * Ly * Lz / 2) % LINK_TILE) return SU_EUNSUPPORTED;
+    }
+    const int Lt = slab ? Lt_loc + 2 : Lt_glob;      // stored time slices
 
     su_lattice* h = new (std::nothrow) su_lattice;
     if (!h) return SU_ENOMEM;
     h->Nc = Nc;
     h->g.L[0] = Lx; h->g.L[1] = Ly; h->g.L[2] = Lz; h->g.L[3] = Lt;
     h->g.Lxh = Lx / 2;
-    h->V = (size_t)Lx * Ly * Lz * Lt;
-    h->g.Vh = (unsigned)(h->V / 2);
-    h->g.Vhp = (unsigned)plane_sites(h->V / 2);
+    const size_t Vstore = (size_t)Lx * Ly * Lz * Lt;
+    h->g.t_halo = slab ? 1 : 0;
+    h->g.Lt_int = slab ? Lt_loc : Lt_glob;
+    h->g.Lt_glob = Lt_glob;
+    h->g.t0g = slab ? (t0 - 1 + Lt_glob) % Lt_glob : 0;
+    h->g.Vsh = (unsigned)((size_t)Lx * Ly * Lz / 2);
+    h->g.Vh_int = h->g.Vsh * (unsigned)h->g.Lt_int;
+    h->V = (size_t)Lx * Ly * Lz * h->g.Lt_int;          // owned sites: what import / export move
+    h->g.Vh = (unsigned)(Vstore / 2);
+    h->g.Vhp = (unsigned)plane_sites(Vstore / 2);
     h->var.store = Nc == 2 ? STORE_QUAT : (o.storage == SU_STORE_RECON12 ? STORE_RECON12 : STORE_FULL);
     h->g.Zc = traversal_z_chunk(h->g, (size_t)elems_per_link(Nc, o.storage) * 2 * (p == SU_FP64 ? 8 : 4));
     h->prec = p;
@@ -274,6 +292,88 @@ su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precis
     if (st == SU_OK && cudaMemset(h->d_counters, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ECUDA;
     if (st != SU_OK) { cudaGetLastError(); su_lattice_destroy(h); return st; }
     *out = h;
+    return SU_OK;
+}
+
+su_status su_lattice_create_ex(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, const su_options* opt,
+                               su_lattice** out) {
+    return create_common(Nc, Lx, Ly, Lz, Lt, false, 0, Lt, p, opt, out);
+}
+
+su_status su_lattice_create_slab(int Nc, int Lx, int Ly, int Lz, int Lt_global, int t0, int Lt_local, su_precision p,
+                                 const su_options* opt, su_lattice** out) {
+    return create_common(Nc, Lx, Ly, Lz, Lt_global, true, t0, Lt_local, p, opt, out);
+}
+
+size_t su_slab_bytes(int Nc, int Lx, int Ly, int Lz, int Lt_local, su_precision p, su_storage s) {
+    if (Lt_local < 2 || (Lt_local & 1)) return 0;
+    return su_lattice_bytes(Nc, Lx, Ly, Lz, Lt_local + 2, p, s);
+}
+
+su_status su_slab_links(su_lattice* h, void** device_links, size_t* bytes) {
+    if (!h || !device_links) return SU_EINVAL;
+    *device_links = h->links;
+    if (bytes) *bytes = h->links_bytes;
+    return SU_OK;
+}
+
+su_status su_slab_set_peers(su_lattice* h, void* device_links_below, void* device_links_above) {
+    if (!h || !device_links_below || !device_links_above) return SU_EINVAL;
+    if (!h->g.t_halo) return fail(h, SU_ESTATE, "su_slab_set_peers on a lattice that is not a slab");
+    DeviceGuard guard(h->device);
+    free_graphs(h);                      // peer pointers are baked into captured launches
+    h->peer_lo = device_links_below; h->peer_hi = device_links_above;
+    return SU_OK;
+}
+
+su_status su_slab_halo_push(su_lattice* h) {
+    if (!h) return SU_EINVAL;
+    if (!h->g.t_halo) return fail(h, SU_ESTATE, "su_slab_halo_push on a lattice that is not a slab");
+    if (!h->peer_lo || !h->peer_hi) return fail(h, SU_ESTATE, "slab lattice: su_slab_set_peers first");
+    if (!h->ready) return fail(h, SU_ESTATE, "su_slab_halo_push before su_init_* / su_import_links");
+    DeviceGuard guard(h->device);
+    // per (mu, parity) plane a time slice is one contiguous range of whole tiles
+    const size_t pair = 2 * (h->prec == SU_FP64 ? 8 : 4);
+    const size_t E = (size_t)elems_per_link(h->Nc, h->var.store == STORE_RECON12 ? SU_STORE_RECON12 : SU_STORE_FULL);
+    const size_t plane = E * h->g.Vhp * pair, slice = E * h->g.Vsh * pair;
+    for (int pl = 0; pl < 8; ++pl) {
+        const char* own = (const char*)h->links + pl * plane;
+        char* lo = (char*)h->peer_lo + pl * plane;
+        char* hi = (char*)h->peer_hi + pl * plane;
+        // first owned slice (stored t = 1) -> upper halo of the slab below (their stored t = Lt_int + 1)
+        SU_CUDA(h, cudaMemcpyAsync(lo + (size_t)(h->g.Lt_int + 1) * slice, own + slice, slice, cudaMemcpyDefault, h->stream), "halo push");
+        // last owned slice (stored t = Lt_int) -> lower halo of the slab above (their stored t = 0)
+        SU_CUDA(h, cudaMemcpyAsync(hi, own + (size_t)h->g.Lt_int * slice, slice, cudaMemcpyDefault, h->stream), "halo push");
+    }
+    return SU_OK;
+}
+
+su_status su_ipc_export(su_lattice* h, unsigned char handle[64]) {
+    if (!h || !handle) return SU_EINVAL;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+    if (!h->owns_links) return fail(h, SU_ESTATE, "su_ipc_export needs a library-owned link buffer (no caller buffer)");
+    DeviceGuard guard(h->device);
+    cudaIpcMemHandle_t m;
+    SU_CUDA(h, cudaIpcGetMemHandle(&m, h->links), "cudaIpcGetMemHandle");
+    memcpy(handle, &m, 64);
+    return SU_OK;
+}
+
+su_status su_ipc_open(su_lattice* h, const unsigned char handle[64], void** device_ptr) {
+    if (!h || !handle || !device_ptr) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    cudaIpcMemHandle_t m;
+    memcpy(&m, handle, 64);
+    void* ptr = nullptr;
+    SU_CUDA(h, cudaIpcOpenMemHandle(&ptr, m, cudaIpcMemLazyEnablePeerAccess), "cudaIpcOpenMemHandle");
+    *device_ptr = ptr;
+    return SU_OK;
+}
+
+su_status su_ipc_close(su_lattice* h, void* device_ptr) {
+    if (!h || !device_ptr) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    SU_CUDA(h, cudaIpcCloseMemHandle(device_ptr), "cudaIpcCloseMemHandle");
     return SU_OK;
 }
 
@@ -322,6 +422,8 @@ su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
     if (!(beta >= 0.0) || !std::isfinite(beta) || n_hb < 0 || n_or < 0 || n_hb > 255)
         return fail(h, SU_EINVAL, "su_sweep: beta must be finite and >= 0, 0 <= n_heatbath <= 255, n_overrelax >= 0");
     if (!h->ready) return fail(h, SU_ESTATE, "su_sweep before su_init_* / su_import_links");
+    if (h->g.t_halo && !(h->peer_lo == h->links && h->peer_hi == h->links))
+        return fail(h, SU_ESTATE, "su_sweep on one slab of several: drive su_substep on all slabs, one sub-step at a time");
     DeviceGuard guard(h->device);
     if (!h->graph_mode) {
         su_status st = enqueue_sweep(h, beta, n_hb, n_or, nullptr, h->timing);
@@ -366,6 +468,7 @@ su_status su_substep(su_lattice* h, double beta, int kind, int pass, int parity,
         parity > 1 || mu < 0 || mu > 3)
         return fail(h, SU_EINVAL, "su_substep: argument out of range");
     if (!h->ready) return fail(h, SU_ESTATE, "su_substep before su_init_* / su_import_links");
+    if (host_attempts && h->g.t_halo) return fail(h, SU_EUNSUPPORTED, "attempt counts are not exported in slab mode");
     DeviceGuard guard(h->device);
     const size_t nsub = (size_t)h->Nc * (h->Nc - 1) / 2, nbytes = nsub * h->g.Vh;
     if (host_attempts) {
@@ -400,6 +503,7 @@ su_status su_plaquette(su_lattice* h, double* out) {
 su_status su_polyakov(su_lattice* h, double out[2]) {
     if (!h || !out) return SU_EINVAL;
     if (!h->ready) return fail(h, SU_ESTATE, "su_polyakov before su_init_* / su_import_links");
+    if (h->g.t_halo) return fail(h, SU_EUNSUPPORTED, "the Polyakov loop crosses slabs: not available in slab mode");
     DeviceGuard guard(h->device);
     AuxArgs a = aux_args(h);
     SU_CUDA(h, SU_BY_NC(h, polyakov_nc, h->var, a, h->stream, &h->n_launch), "polyakov kernels");

@@ -45,25 +45,44 @@ template <class T> __device__ __forceinline__ void mad_ca(cx<T>& acc, cx<T> a, c
 constexpr int LINK_TILE = 32;   // sites per AoSoA tile of the link storage (one warp-wide row per matrix element)
 
 struct Geom {
-    int L[4];
+    int L[4];       // extents of the STORED lattice; L[3] includes the two halo time slices in slab mode
     int Lxh;        // Lx / 2
-    unsigned Vh;    // V / 2 = sites per parity
+    unsigned Vh;    // stored sites per parity
     unsigned Vhp;   // Vh rounded up to a multiple of LINK_TILE = sites per stored plane
     int Zc;         // z-chunk of the update kernel's traversal order (divides Lz)
+    // t-slab decomposition: the handle owns Lt_int time slices of a global lattice of
+    // Lt_glob slices and stores one halo slice below and above them (t_halo = 1). Without it: t_halo = 0,
+    // Lt_int = L[3] = Lt_glob, t0g = 0 and the t direction wraps periodically inside the buffer.
+    int t_halo;     // 0 or 1
+    int Lt_int;     // interior (owned) time slices
+    int Lt_glob;    // global time extent
+    int t0g;        // global t of stored slice 0, in [0, Lt_glob)
+    unsigned Vh_int;   // interior sites per parity = Lx Ly Lz Lt_int / 2
+    unsigned Vsh;      // sites per parity of one time slice = Lx Ly Lz / 2
 };
+
+// parity of a stored site = parity of its GLOBAL coordinates (Lt_glob is even)
+__device__ __forceinline__ int site_parity(const Geom& g, int x, int y, int z, int t_store) {
+    return (x + y + z + t_store + g.t0g) & 1;
+}
+__device__ __forceinline__ int global_t(const Geom& g, int t_store) {
+    const int t = t_store + g.t0g;             // can reach 2 Lt_glob (a single slab's upper halo)
+    return t < g.Lt_glob ? t : t % g.Lt_glob;
+}
 
 __device__ __forceinline__ void decode_cb(const Geom& g, unsigned cb, int parity, int c[4]) {
     unsigned xh = cb % (unsigned)g.Lxh, r = cb / (unsigned)g.Lxh;
     c[1] = (int)(r % (unsigned)g.L[1]); r /= (unsigned)g.L[1];
     c[2] = (int)(r % (unsigned)g.L[2]);
     c[3] = (int)(r / (unsigned)g.L[2]);
-    c[0] = 2 * (int)xh + ((c[1] + c[2] + c[3] + parity) & 1);
+    c[0] = 2 * (int)xh + ((c[1] + c[2] + c[3] + g.t0g + parity) & 1);
 }
 __device__ __forceinline__ unsigned cb_of(const Geom& g, int x, int y, int z, int t) {
     return (unsigned)(x >> 1) + (unsigned)g.Lxh * ((unsigned)y + (unsigned)g.L[1] * ((unsigned)z + (unsigned)g.L[2] * (unsigned)t));
 }
+// lexicographic index of a stored site in the GLOBAL lattice (the RNG counter word c0)
 __device__ __forceinline__ unsigned lex_of(const Geom& g, const int c[4]) {
-    return (unsigned)c[0] + (unsigned)g.L[0] * ((unsigned)c[1] + (unsigned)g.L[1] * ((unsigned)c[2] + (unsigned)g.L[2] * (unsigned)c[3]));
+    return (unsigned)c[0] + (unsigned)g.L[0] * ((unsigned)c[1] + (unsigned)g.L[1] * ((unsigned)c[2] + (unsigned)g.L[2] * (unsigned)global_t(g, c[3])));
 }
 // checkerboard index of c + s1*e_{d1} + s2*e_{d2} (s in {-1,0,+1}), periodic wrap
 __device__ __forceinline__ unsigned cb_shift(const Geom& g, const int c[4], int d1, int s1, int d2 = 0, int s2 = 0) {

@@ -24,12 +24,20 @@ struct UpdateArgs {
     const uint32_t* sweep_ptr;         // device; when non-NULL the sweep counter is read from here (graph replay)
     uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
     unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
+    // slab mode: link buffers of the slabs below / above in t (peer memory over NVLink, or this device). The
+    // kernel that updates a link of the first / last owned slice also stores it into that neighbour's halo.
+    void* peer_lo;
+    void* peer_hi;
 };
+
+// checkerboard index, in the neighbour's buffer, of the halo copy of an edge site (all slabs have Lt_int slices)
+__device__ __forceinline__ unsigned halo_cb_lo(const Geom& g, unsigned cb) { return cb + (unsigned)g.Lt_int * g.Vsh; }   // -> their upper halo
+__device__ __forceinline__ unsigned halo_cb_hi(const Geom& g, unsigned cb) { return cb - (unsigned)g.Lt_int * g.Vsh; }   // -> their lower halo
 
 // The site a thread works on and the checkerboard-index offsets of its 8 neighbours.
 struct SiteNbr {
-    unsigned cb;        // checkerboard index of x
-    uint32_t lex;       // lexicographic site index of x (RNG counter word c0)
+    unsigned cb;        // checkerboard index of x in the stored lattice
+    uint32_t lex;       // lexicographic index of x in the global lattice (RNG counter word c0)
     int dp[4], dm[4];   // cb(x + e_d) - cb(x), cb(x - e_d) - cb(x)   (periodic)
 };
 
@@ -37,28 +45,42 @@ __device__ __forceinline__ int sel4(int i, int v0, int v1, int v2, int v3) {
     return i == 0 ? v0 : (i == 1 ? v1 : (i == 2 ? v2 : v3));
 }
 
-// traversal index -> site; all indices stay in registers (no dynamically indexed arrays)
+// traversal index (over the OWNED sites of one parity) -> site; all indices stay in registers
 __device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int parity, SiteNbr& s) {
     const unsigned row = (unsigned)g.Lxh, pl = row * (unsigned)g.L[1];
-    const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.L[3];
+    const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
     const unsigned zc = tix / span;  unsigned r = tix - zc * span;
-    const unsigned t = r / grp;      r -= t * grp;
+    const unsigned ti = r / grp;     r -= ti * grp;
     const unsigned zi = r / pl;      r -= zi * pl;
     const unsigned y = r / row;
     const unsigned xh = r - y * row;
     const unsigned z = zc * (unsigned)g.Zc + zi;
+    const unsigned t = ti + (unsigned)g.t_halo;                          // stored time slice
     const int sy = (int)row, sz = (int)pl, st = (int)(pl * (unsigned)g.L[2]);
-    const int q = (int)((y + z + t + (unsigned)parity) & 1u);          // x = 2 xh + q
+    const int q = (int)((y + z + t + (unsigned)g.t0g + (unsigned)parity) & 1u);          // x = 2 xh + q
     s.cb = xh + row * (y + (unsigned)g.L[1] * (z + (unsigned)g.L[2] * t));
-    s.lex = 2u * s.cb + (unsigned)q;
+    s.lex = 2u * (xh + row * (y + (unsigned)g.L[1] * (z + (unsigned)g.L[2] * (unsigned)global_t(g, (int)t)))) + (unsigned)q;
     s.dp[0] = q ? ((int)xh + 1 == g.Lxh ? 1 - g.Lxh : 1) : 0;
     s.dm[0] = q ? 0 : (xh == 0 ? g.Lxh - 1 : -1);
     s.dp[1] = ((int)y + 1 == g.L[1]) ? -(g.L[1] - 1) * sy : sy;
     s.dm[1] = (y == 0) ? (g.L[1] - 1) * sy : -sy;
     s.dp[2] = ((int)z + 1 == g.L[2]) ? -(g.L[2] - 1) * sz : sz;
     s.dm[2] = (z == 0) ? (g.L[2] - 1) * sz : -sz;
-    s.dp[3] = ((int)t + 1 == g.L[3]) ? -(g.L[3] - 1) * st : st;
-    s.dm[3] = (t == 0) ? (g.L[3] - 1) * st : -st;
+    if (g.t_halo) {             // the neighbours in t are the halo slices: no wrap inside the buffer
+        s.dp[3] = st; s.dm[3] = -st;
+    } else {
+        s.dp[3] = ((int)t + 1 == g.L[3]) ? -(g.L[3] - 1) * st : st;
+        s.dm[3] = (t == 0) ? (g.L[3] - 1) * st : -st;
+    }
+}
+
+// slab mode: 1 = the thread's site lies in the first owned time slice, 2 = in the last one, 0 otherwise.
+// Recomputed from the traversal index at store time so that nothing stays live across the kernel body.
+__device__ __forceinline__ int slab_edge(const Geom& g, unsigned tix) {
+    if (!g.t_halo) return 0;
+    const unsigned grp = (unsigned)g.Lxh * (unsigned)g.L[1] * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
+    const unsigned ti = (tix % span) / grp;
+    return (ti == 0 ? 1 : 0) | ((int)ti + 1 == g.Lt_int ? 2 : 0);
 }
 
 // FUSE3: each staple term S += A B C (three links) is evaluated row by row with all three operands
@@ -70,7 +92,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
     typedef Mat<NC, T, UNR> M;
     typedef cx<T> C;
     const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = tix < a.g.Vh;
+    const bool active = tix < a.g.Vh_int;
     unsigned att_total = 0, exhausted = 0;
     if (active) {
         const int p = a.parity, mu = a.mu;
@@ -126,6 +148,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
                                            a.attempts ? a.attempts + cb : nullptr, (size_t)a.g.Vh,
                                            att_total, exhausted);
         IO::template store<true>(pl_self, cb, U);
+        if (const int edge = slab_edge(a.g, tix)) {          // fused halo push (slab mode only)
+            if (edge & 1) IO::template store<true>(IO::plane(a.peer_lo, a.g, mu, p), halo_cb_lo(a.g, cb), U);
+            if (edge & 2) IO::template store<true>(IO::plane(a.peer_hi, a.g, mu, p), halo_cb_hi(a.g, cb), U);
+        }
     }
     if (KIND == KIND_HB) {
         for (int o = 16; o > 0; o >>= 1) {
@@ -159,11 +185,10 @@ template <class T, int KIND, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) {
     typedef typename V2<T>::type T2;
     const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = tix < a.g.Vh;
+    const bool active = tix < a.g.Vh_int;
     unsigned att_total = 0, exhausted = 0;
     if (active) {
         const int p = a.parity, mu = a.mu;
-        const unsigned Vh = a.g.Vh;
         SiteNbr s;
         site_of_thread(a.g, tix, p, s);
         const unsigned cb = s.cb;
@@ -223,6 +248,17 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
             T2* q = pl_self + qsite<T>(cb);
             stg2<T, true>(q, V2<T>::make(P[0], P[1]));
             stg2<T, true>(q + LINK_TILE, V2<T>::make(P[2], P[3]));
+            if (const int edge = slab_edge(a.g, tix)) {      // fused halo push (slab mode only)
+                const size_t plane_off = (size_t)(mu * 2 + p) * 2 * a.g.Vhp;
+                if (edge & 1) {
+                    T2* h = (T2*)a.peer_lo + plane_off + qsite<T>(halo_cb_lo(a.g, cb));
+                    stg2<T, true>(h, V2<T>::make(P[0], P[1])); stg2<T, true>(h + LINK_TILE, V2<T>::make(P[2], P[3]));
+                }
+                if (edge & 2) {
+                    T2* h = (T2*)a.peer_hi + plane_off + qsite<T>(halo_cb_hi(a.g, cb));
+                    stg2<T, true>(h, V2<T>::make(P[0], P[1])); stg2<T, true>(h + LINK_TILE, V2<T>::make(P[2], P[3]));
+                }
+            }
         }
     }
     if (KIND == KIND_HB) {

@@ -23,10 +23,10 @@ template <int BLOCK_, int MINB_, bool FUSE3_ = false, bool KUNR_ = false> struct
 template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB>
 static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t st) {
     if (kind == KIND_HB) {
-        const unsigned grid = (a.g.Vh + HB::BLOCK - 1) / HB::BLOCK;
+        const unsigned grid = (a.g.Vh_int + HB::BLOCK - 1) / HB::BLOCK;
         k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR><<<grid, HB::BLOCK, 0, st>>>(a);
     } else {
-        const unsigned grid = (a.g.Vh + OR::BLOCK - 1) / OR::BLOCK;
+        const unsigned grid = (a.g.Vh_int + OR::BLOCK - 1) / OR::BLOCK;
         k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR><<<grid, OR::BLOCK, 0, st>>>(a);
     }
     return cudaGetLastError();
@@ -81,7 +81,7 @@ cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateA
 #if SUG_NC == 2
     if (!v.generic) {
         constexpr int BLOCK = 128;
-        const unsigned grid = (a.g.Vh + BLOCK - 1) / BLOCK;
+        const unsigned grid = (a.g.Vh_int + BLOCK - 1) / BLOCK;
         if (f64) { if (kind == KIND_HB) k_update_su2<double, KIND_HB, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); else k_update_su2<double, KIND_OR, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); }
         else     { if (kind == KIND_HB) k_update_su2<float,  KIND_HB, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); else k_update_su2<float,  KIND_OR, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); }
         return cudaGetLastError();

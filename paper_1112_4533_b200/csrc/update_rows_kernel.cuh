@@ -12,7 +12,7 @@
 //                   -> same numbers) and rotate their own row (eq 15); subgroups on disjoint row pairs
 //                   commute exactly, so the lexicographic sequence runs as a wavefront of 2 Nc - 3 slots.
 // A warp holds floor(32 / Nc) links; left-over lanes shadow the last group and never store.
-// The order of operations inside every sum is the one of update_kernel.cuh and of the oracle.
+// The order of operations inside every sum is the one of update_kernel.cuh (products left to right).
 #pragma once
 #include "update_kernel.cuh"
 
@@ -57,8 +57,8 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value) k_update_rows(co
     const int r = shadow ? lane - LPW * NC : lane - g * NC;   // row owned by this lane
     const int gbase = g * NC;                                 // first lane of the group
     unsigned tix = (blockIdx.x * WARPS + (unsigned)warp) * LPW + (unsigned)g;
-    const bool owner = !shadow && tix < a.g.Vh;               // lanes past the end redo the last link, never store
-    if (tix >= a.g.Vh) tix = a.g.Vh - 1;
+    const bool owner = !shadow && tix < a.g.Vh_int;           // lanes past the end redo the last link, never store
+    if (tix >= a.g.Vh_int) tix = a.g.Vh_int - 1;
     C(*M)[STRIDE] = stage[warp * LPW + g];
 
     const int p = a.parity, mu = a.mu;
@@ -215,6 +215,18 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value) k_update_rows(co
         T2* q = IO::site(pl_self, cb) + (size_t)r * NC * LINK_TILE;
 #pragma unroll
         for (int c = 0; c < NC; ++c) __stcs(q + c * LINK_TILE, V2<T>::make(U[c].re, U[c].im));
+        if (const int edge = slab_edge(a.g, tix)) {          // fused halo push (slab mode only)
+            if (edge & 1) {
+                T2* h = IO::site(IO::plane(a.peer_lo, a.g, mu, p), halo_cb_lo(a.g, cb)) + (size_t)r * NC * LINK_TILE;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) __stcs(h + c * LINK_TILE, V2<T>::make(U[c].re, U[c].im));
+            }
+            if (edge & 2) {
+                T2* h = IO::site(IO::plane(a.peer_hi, a.g, mu, p), halo_cb_hi(a.g, cb)) + (size_t)r * NC * LINK_TILE;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) __stcs(h + c * LINK_TILE, V2<T>::make(U[c].re, U[c].im));
+            }
+        }
     }
     if (KIND == KIND_HB) {
         for (int o = 16; o > 0; o >>= 1) {
@@ -232,7 +244,7 @@ template <int NC, class T>
 static cudaError_t launch_update_rows(int kind, const UpdateArgs& a, cudaStream_t st) {
     constexpr int WARPS = RowsWarps<NC, T>::value;
     const unsigned per_block = (unsigned)(WARPS * RowsCfg<NC>::LPW);
-    const unsigned grid = (a.g.Vh + per_block - 1) / per_block;
+    const unsigned grid = (a.g.Vh_int + per_block - 1) / per_block;
     if (kind == KIND_HB) k_update_rows<NC, T, KIND_HB><<<grid, 32 * WARPS, 0, st>>>(a);
     else                 k_update_rows<NC, T, KIND_OR><<<grid, 32 * WARPS, 0, st>>>(a);
     return cudaGetLastError();
