@@ -308,6 +308,61 @@ def run_reference(args, wl, rank):
     return 0
 
 
+def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
+    """--parallel slabs: ONE lattice, rank r owns the time slices [r Lt/N, (r+1) Lt/N). Step =
+    40 sub-steps (each followed by the stream-ordered rank ordering) + reunitarise + plaquette (all-reduce). The
+    Polyakov loop crosses slabs and is not part of this mode's step. Strong scaling: total work fixed."""
+    from paper_1112_4533_b200.slab import DistributedLattice
+    D = DistributedLattice(wl["Nc"], (wl["L"],) * 4, args.precision, recon12, args.kernel, device=local)
+    (D.init_hot if wl["start"] == "hot" else D.init_cold)(wl["seed"])
+    reunit = wl["Nc"] > 2
+
+    def step():
+        D.sweep(wl["beta"], N_HB, N_OR)
+        if reunit:
+            D.reunitarize()
+        return D.plaquette()
+
+    for _ in range(warmup):
+        step()
+    n0 = D.lat.launch_count()
+    dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    ev0.record(D.lat.stream)
+    for _ in range(args.steps):
+        plaq = step()
+    ev1.record(D.lat.stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    dist.barrier()
+    ms = max_over_ranks(dist, ev0.elapsed_time(ev1), "cuda")
+    clocks = sampler.stop(t0, t1)
+    launches = D.lat.launch_count() - n0
+    updates_step = (N_HB + N_OR) * 4 * wl["L"] ** 4                  # the whole lattice, once
+    if rank == 0:
+        line = {"metric": METRIC, "value": whole_job_rate(1, updates_step, ms, args.steps), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32",
+                "data": "synthetic",
+                "config": {"workload": args.workload, "Nc": wl["Nc"], "lattice": f"{wl['L']}^4", "beta": wl["beta"],
+                           "start": f"{wl['start']} (Philox seed {wl['seed']})", "sweep": "1 heatbath + 4 overrelaxation",
+                           "step": "40 x (su_substep + rank ordering) + su_reunitarize + su_plaquette (all-reduce)",
+                           "storage": args.storage, "kernel": args.kernel,
+                           "parallelism": f"{world} t-slabs of {wl['L'] // world} time slices, halo push fused into the "
+                                          "update kernel (peer memory), ordering by a 1-element all-reduce",
+                           "l2": "inputs larger than L2 (no flush)"},
+                "roofline": None, "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
+                "plaquette": plaq}
+        print(json.dumps(line), flush=True)
+    D.close()
+    dist.barrier()
+    dist.destroy_process_group()
+    return 0
+
+
 def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
     """Turn one timed run into the metric, GFLOPS and the roofline object of its dominant (OR) kernel."""
     Nc, V = wl["Nc"], wl["L"] ** 4
@@ -343,6 +398,9 @@ def main():
     ap.add_argument("--storage", default="full", choices=["full", "recon12"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "specialised", "generic"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default; weak scaling) or ONE lattice cut into N t-slabs with "
+                         "halo pushes over peer memory (strong scaling; DESIGN.md 9)")
     ap.add_argument("--no-variants", action="store_true", help="skip the extra fp32 / 12-real runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -367,6 +425,13 @@ def main():
     warmup = max(args.warmup, 3)
     peak = measured_peaks()
     recon12 = args.storage == "recon12"
+    if args.parallel == "slabs":
+        if dist is None:                          # a single rank still goes through the slab path (one slab, self-peered)
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29533")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
+        return run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12)
 
     def timed(precision, r12, kernel, steps, wu, clocks):
         lat = make_lattice(su, wl, precision, r12, kernel, rank, local)
