@@ -18,6 +18,13 @@
 
 namespace sug {
 
+#ifndef SUG_ROWS_MINB
+#define SUG_ROWS_MINB 4
+#endif
+#ifndef SUG_ROWS_MAXW
+#define SUG_ROWS_MAXW 4
+#endif
+
 template <int NC> struct RowsCfg {
     static constexpr int LPW = 32 / NC;                       // links per warp
     static constexpr int STRIDE = NC * NC + 1;                // complex elements per staged matrix (+1: bank spread)
@@ -27,7 +34,8 @@ template <int NC> struct RowsCfg {
 // warps per block: as many (<= 4) as keep NB staged matrices per link within 48 KB of static shared memory
 template <int NC, class T, int NB = RowsCfg<NC>::NBUF> struct RowsWarps {
     static constexpr size_t LIM = 48 * 1024, R = sizeof(T);
-    static constexpr int value = RowsCfg<NC>::bytes(4, R, NB) <= LIM ? 4 : (RowsCfg<NC>::bytes(3, R, NB) <= LIM ? 3 : (RowsCfg<NC>::bytes(2, R, NB) <= LIM ? 2 : 1));
+    static constexpr int fit = RowsCfg<NC>::bytes(4, R, NB) <= LIM ? 4 : (RowsCfg<NC>::bytes(3, R, NB) <= LIM ? 3 : (RowsCfg<NC>::bytes(2, R, NB) <= LIM ? 2 : 1));
+    static constexpr int value = fit < SUG_ROWS_MAXW ? fit : SUG_ROWS_MAXW;
 };
 
 template <class T> __device__ __forceinline__ cx<T> shfl_cx(cx<T> v, int src) {
@@ -42,7 +50,7 @@ template <int NC, class T> __device__ __forceinline__ cx<T> row_pick(const cx<T>
 }
 
 template <int NC, class T, int KIND>
-__global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value) k_update_rows(const UpdateArgs a) {
+__global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k_update_rows(const UpdateArgs a) {
     typedef RowsCfg<NC> Cfg;
     typedef LinkIO<NC, T, STORE_FULL, true> IO;
     typedef typename IO::T2 T2;
