@@ -308,6 +308,42 @@ def run_reference(args, wl, rank):
     return 0
 
 
+def run_nc_scan(args, torch, su, local):
+    """One JSON line per (Nc, kernel, lattice, precision): ms per iteration, the paper's iteration:
+    1 heatbath + 1 overrelaxation + reunitarisation (Nc >= 3) + plaquette, cold start, CUDA-graph replay of the sweep."""
+    rows = []
+    for L in (8, 16):
+        for precision in ("fp32", "fp64"):
+            for Nc in range(2, su.SU_MAX_NC + 1):
+                for kernel in (("specialised", "generic") if Nc <= 4 else ("generic",)):
+                    lat = su.Lattice(Nc, (L,) * 4, precision, kernel=kernel, device=local, graph=True)
+                    lat.init_cold(1)
+
+                    def it():
+                        lat.sweep(6.2, 1, 1)
+                        if Nc > 2:
+                            lat.reunitarize()
+                        return lat.plaquette()
+
+                    for _ in range(5):
+                        it()
+                    torch.cuda.synchronize()
+                    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    n = max(5, args.steps)
+                    ev0.record(lat.stream)
+                    for _ in range(n):
+                        plaq = it()
+                    ev1.record(lat.stream)
+                    torch.cuda.synchronize()
+                    ms = ev0.elapsed_time(ev1) / n
+                    rows.append({"scan": "nc", "Nc": Nc, "kernel": kernel, "lattice": f"{L}^4", "precision": precision,
+                                 "beta": 6.2, "iteration": "1 HB + 1 OR + reunitarise + plaquette", "ms_per_iteration": ms,
+                                 "link_updates_per_s": 2 * 4 * L ** 4 / (ms * 1e-3), "plaquette": plaq})
+                    print(json.dumps(rows[-1]), flush=True)
+                    lat.close()
+    return 0
+
+
 def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
     """--parallel slabs: ONE lattice, rank r owns the time slices [r Lt/N, (r+1) Lt/N). Step =
     40 sub-steps (each followed by the stream-ordered rank ordering) + reunitarise + plaquette (all-reduce). The
@@ -401,6 +437,9 @@ def main():
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: independent replicas (default; weak scaling) or ONE lattice cut into N t-slabs with "
                          "halo pushes over peer memory (strong scaling; DESIGN.md 9)")
+    ap.add_argument("--nc-scan", action="store_true",
+                    help="the paper's Nc-scaling study (PAPER.md:295-303, Figs 11-12): time per iteration (1 heatbath + 1 "
+                         "overrelaxation + reunitarise + plaquette) vs Nc at 8^4 and 16^4, beta 6.2, generic and specialised")
     ap.add_argument("--no-variants", action="store_true", help="skip the extra fp32 / 12-real runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -425,6 +464,8 @@ def main():
     warmup = max(args.warmup, 3)
     peak = measured_peaks()
     recon12 = args.storage == "recon12"
+    if args.nc_scan:
+        return run_nc_scan(args, torch, su, local)
     if args.parallel == "slabs":
         if dist is None:                          # a single rank still goes through the slab path (one slab, self-peered)
             import torch.distributed as dist
