@@ -308,6 +308,95 @@ __device__ __forceinline__ bool link_of_thread(const Geom& g, unsigned idx, int&
     return true;
 }
 
+// Reunitarisation, row-per-lane (generic path): modified Gram-Schmidt over the rows with the finished row
+// broadcast by warp shuffle, then the determinant by Gaussian elimination with partial pivoting distributed
+// over the lanes (the pivot row is the unused lane with the largest |M_rc|^2; no rows are swapped, the sign is
+// the parity of the pivot order), last row *= conj(det)/|det| (reading R10). Same formulas as
+// gram_schmidt_rows / determinant, which the thread-per-link kernel runs on local arrays.
+template <int NC, class T>
+__global__ void __launch_bounds__(128) k_reunit_rows(const AuxArgs a) {
+    typedef RowsCfg<NC> Cfg;
+    typedef LinkIO<NC, T, STORE_FULL, true> IO;
+    typedef typename IO::T2 T2;
+    typedef cx<T> C;
+    constexpr int LPW = Cfg::LPW;
+    const int lane = (int)(threadIdx.x & 31u), warp = (int)(threadIdx.x >> 5);
+    const bool shadow = lane >= LPW * NC;
+    const int g = shadow ? LPW - 1 : lane / NC;
+    const int r = shadow ? lane - LPW * NC : lane - g * NC;
+    const int gbase = g * NC;
+    const unsigned nlinks = 8u * a.g.Vh;
+    unsigned idx = (blockIdx.x * 4u + (unsigned)warp) * LPW + (unsigned)g;
+    const bool owner = !shadow && idx < nlinks;
+    if (idx >= nlinks) idx = nlinks - 1;
+    int mu, p; unsigned cb;
+    link_of_thread(a.g, idx, mu, p, cb);
+    T2* q = IO::site(IO::plane(a.links, a.g, mu, p), cb) + (size_t)r * NC * LINK_TILE;
+    C U[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) { T2 v = __ldcs(q + c * LINK_TILE); U[c] = mk<T>(v.x, v.y); }
+    // modified Gram-Schmidt, rows top to bottom
+#pragma unroll 1
+    for (int pr = 0; pr < NC; ++pr) {
+        T n2 = 0;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) n2 += U[k].re * U[k].re + U[k].im * U[k].im;
+        const T inv = (T)1 / Fn<T>::sqrt(n2);
+        if (r == pr) {
+#pragma unroll
+            for (int k = 0; k < NC; ++k) U[k] = inv * U[k];
+        }
+        C dot = mk<T>(0, 0), row[NC];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) { row[k] = shfl_cx(U[k], gbase + pr); mad_ca(dot, row[k], U[k]); }
+        if (r > pr) {
+#pragma unroll
+            for (int k = 0; k < NC; ++k) U[k] = U[k] - dot * row[k];
+        }
+    }
+    // determinant
+    C M[NC];
+#pragma unroll
+    for (int k = 0; k < NC; ++k) M[k] = U[k];
+    C det = mk<T>(1, 0);
+    bool used = false, odd = false;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        const T mag = used ? (T)-1 : M[c].re * M[c].re + M[c].im * M[c].im;
+        T best = (T)-1;
+        int pl = 0;
+#pragma unroll
+        for (int l = 0; l < NC; ++l) {
+            const T ml = __shfl_sync(0xffffffffu, mag, gbase + l);
+            if (ml > best) { best = ml; pl = l; }
+        }
+        const unsigned unused = (__ballot_sync(0xffffffffu, !used) >> gbase) & ((1u << NC) - 1u);
+        if (__popc(unused & ((1u << pl) - 1u)) & 1) odd = !odd;      // unused rows above the pivot row = inversions
+        C piv[NC];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) piv[k] = shfl_cx(M[k], gbase + pl);
+        det = det * piv[c];
+        const C pinv = ((T)1 / best) * conj(piv[c]);
+        if (r == pl) used = true;
+        if (!used) {
+            const C f = M[c] * pinv;
+#pragma unroll
+            for (int k = c; k < NC; ++k) M[k] = M[k] - f * piv[k];
+        }
+    }
+    if (odd) det = mk<T>(-det.re, -det.im);
+    const T dinv = (T)1 / Fn<T>::sqrt(det.re * det.re + det.im * det.im);
+    const C ph = mk<T>(det.re * dinv, -det.im * dinv);
+    if (r == NC - 1) {
+#pragma unroll
+        for (int k = 0; k < NC; ++k) U[k] = U[k] * ph;
+    }
+    if (owner) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) __stcs(q + c * LINK_TILE, V2<T>::make(U[c].re, U[c].im));
+    }
+}
+
 // SU(3) rows 0,1 by modified Gram-Schmidt in registers (same operation order as gram_schmidt_rows)
 template <class T>
 __device__ __forceinline__ void gram_schmidt_su3_two_rows(cx<T>* U) {
@@ -548,6 +637,17 @@ cudaError_t SUG_CAT(polyakov_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cud
 }
 
 cudaError_t SUG_CAT(reunit_nc, SUG_NC)(const Variant& v, const AuxArgs& a, cudaStream_t st, uint64_t* n_launch) {
+#if SUG_NC >= 5
+    if (use_rows(v)) {          // Nc <= 4 already reunitarise in registers, one thread per link
+        constexpr int NC = SUG_NC;
+        const unsigned per_block = 4u * RowsCfg<NC>::LPW;
+        const unsigned grid_r = (8u * a.g.Vh + per_block - 1) / per_block;
+        if (v.prec == SU_FP64) k_reunit_rows<NC, double><<<grid_r, 128, 0, st>>>(a);
+        else                   k_reunit_rows<NC, float><<<grid_r, 128, 0, st>>>(a);
+        ++*n_launch;
+        return cudaGetLastError();
+    }
+#endif
     const unsigned grid = (8u * a.g.Vh + 127u) / 128u;
     SUG_AUX_DISPATCH(k_reunit, grid, 128);
     return cudaGetLastError();
