@@ -353,9 +353,24 @@ template <> struct Fn<double> {
 // always the fp64 one, and the accepted attempt's lambda^2 is then evaluated in fp64 once, after the
 // loop, by the whole warp together (a warp would otherwise run the fp64 log/log/cos body for every
 // attempt any of its lanes needs: 1.9 times per draw at beta = 6 instead of once).
+// Direction of the heatbath vector: a point uniform on the unit sphere from the "direction"
+// Philox block of the draw. It does not depend on the links, so a kernel may evaluate it ahead of the
+// staple (in the shadow of the first loads) and hand it to kp_draw.
+template <class T>
+__device__ __forceinline__ void kp_direction(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2_base, T n[3]) {
+    uint32_t d[4];
+    philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_DIR << 28), 0u, k0, k1, d);
+    const T u1 = uniform01<T>(d[0]), u2 = uniform01<T>(d[1]);
+    const T cos_t = (T)1 - (T)2 * u1;
+    const T sin_t = Fn<T>::sqrt(Fn<T>::max0((T)1 - cos_t * cos_t));
+    T sp, cp;
+    Fn<T>::sincos2pi(u2, &sp, &cp);
+    n[0] = sin_t * cp; n[1] = sin_t * sp; n[2] = cos_t;
+}
+
 template <class T>
 __device__ __forceinline__ int kp_draw(T alpha, T m_inv2a, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
-                                       uint32_t c2_base, T v[4]) {
+                                       uint32_t c2_base, T v[4], const T* dir = nullptr, int dir_stride = 0) {
     if (!(alpha > (T)0) || !Fn<T>::finite(alpha)) return 0;
     constexpr bool PRETEST = (sizeof(T) == 8) && (SUG_KP_PRETEST != 0);
     const float two_af = 2.0f * (float)alpha;
@@ -391,15 +406,11 @@ __device__ __forceinline__ int kp_draw(T alpha, T m_inv2a, uint32_t k0, uint32_t
         T lambda2 = (Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) * m_inv2a;
         a0 = (T)1 - (T)2 * lambda2;
     }
-    uint32_t d[4];
-    philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_DIR << 28), 0u, k0, k1, d);
-    T u1 = uniform01<T>(d[0]), u2 = uniform01<T>(d[1]);
-    T cos_t = (T)1 - (T)2 * u1;
-    T sin_t = Fn<T>::sqrt(Fn<T>::max0((T)1 - cos_t * cos_t));
-    T rho = Fn<T>::sqrt(Fn<T>::max0((T)1 - a0 * a0));
-    T sp, cp;
-    Fn<T>::sincos2pi(u2, &sp, &cp);
-    v[0] = a0; v[1] = rho * sin_t * cp; v[2] = rho * sin_t * sp; v[3] = rho * cos_t;
+    T n[3];
+    if (dir) { n[0] = dir[0]; n[1] = dir[dir_stride]; n[2] = dir[2 * dir_stride]; }
+    else kp_direction<T>(k0, k1, c0, c1, c2_base, n);
+    const T rho = Fn<T>::sqrt(Fn<T>::max0((T)1 - a0 * a0));
+    v[0] = a0; v[1] = rho * n[0]; v[2] = rho * n[1]; v[3] = rho * n[2];
     return used;
 }
 
@@ -421,7 +432,8 @@ template <int NC, class T, int KIND, bool UNR>
 __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uint32_t k0, uint32_t k1,
                                                  uint32_t c0, uint32_t c1, uint32_t c2_base,
                                                  uint8_t* att_out, size_t att_stride,
-                                                 unsigned& att_total, unsigned& exhausted) {
+                                                 unsigned& att_total, unsigned& exhausted,
+                                                 const T* dirs = nullptr, int dir_stride = 0) {
     int q = 0;
     const T two_beta_over_nc = (T)2 * beta / (T)NC;      // alpha = 2 beta k / Nc (reading R3)
     const T m_nc_over_4beta = (T)-0.25 * (T)NC / beta;   // -1 / (2 alpha) = this / k   (heatbath only)
@@ -442,7 +454,7 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                     T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                     T v[4];
                     used = kp_draw<T>(two_beta_over_nc * k, m_nc_over_4beta * ik, k0, k1, c0, c1,
-                                      c2_base | (uint32_t)q, v);
+                                      c2_base | (uint32_t)q, v, dirs ? dirs + 3 * q * dir_stride : nullptr, dir_stride);
                     if (used) quat_mul(v, ud, a); else ok = false;
                 } else {
                     // a = (u~^dagger)^2 = conj(r)^2 / k^2 (eq 17): no square root, one reciprocal

@@ -15,6 +15,13 @@
 
 namespace sug {
 
+#ifndef SUG_TMINUS_STREAM
+#define SUG_TMINUS_STREAM 1
+#endif
+#ifndef SUG_KP_PREDIR
+#define SUG_KP_PREDIR 1
+#endif
+
 struct UpdateArgs {
     void* links;
     Geom g;
@@ -101,6 +108,21 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
         const unsigned cb = s.cb;
         const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
 
+        // heatbath, register kernels: the directions of all subgroup draws are link-independent; evaluate them
+        // now, in the shadow of the first loads, and park them in shared memory (one private column per thread)
+        constexpr int NSUB = NC * (NC - 1) / 2;
+        constexpr bool PREDIR = (KIND == KIND_HB) && UNR && SUG_KP_PREDIR && sizeof(T) == 4;   // fp32 only: measured -2.7 % (fp64: +5 %)
+        __shared__ T dir_sm[PREDIR ? 3 * NSUB : 1][PREDIR ? BLOCK : 1];
+        const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
+        if (PREDIR) {
+#pragma unroll
+            for (int q = 0; q < NSUB; ++q) {
+                T n[3];
+                kp_direction<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2(0, (int)a.pass, p, mu, q), n);
+                dir_sm[3 * q][threadIdx.x] = n[0]; dir_sm[3 * q + 1][threadIdx.x] = n[1]; dir_sm[3 * q + 2][threadIdx.x] = n[2];
+            }
+        }
+
         C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
         M::zero(S);
         const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
@@ -118,9 +140,17 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
                 IO::template load<LD_RO>(pl_nu_s, cb, A);
                 M::acc_nnd(S, A, B, P);
                 // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
-                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
-                IO::template load<LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
-                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
+                if (SUG_TMINUS_STREAM && k == 2 && nu == 3) {
+                    // links of the time slice below: with the traversal walking up in t this is their last
+                    // use in the sub-step, so they are fetched evict-first and leave L2 to the slices ahead
+                    IO::template load<LD_STREAM>(pl_mu_o, cb + (unsigned)dmnu, B);
+                    IO::template load<LD_STREAM>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                    IO::template load<LD_STREAM>(pl_nu_o, cb + (unsigned)dmnu, A);
+                } else {
+                    IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
+                    IO::template load<LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                    IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
+                }
                 M::acc_dnn(S, A, B, P);
             } else {
                 // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
@@ -142,11 +172,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
         C* W = B;
         IO::template load<LD_STREAM>(pl_self, cb, U);
         M::mul_nd(U, S, W);                                   // W = U S^dagger
-        update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex,
-                                           a.sweep_ptr ? *a.sweep_ptr : a.sweep,
+        update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex, sweep_ctr,
                                            pack_c2(0, (int)a.pass, p, mu, 0),
                                            a.attempts ? a.attempts + cb : nullptr, (size_t)a.g.Vh,
-                                           att_total, exhausted);
+                                           att_total, exhausted,
+                                           PREDIR ? &dir_sm[0][threadIdx.x] : nullptr, PREDIR ? BLOCK : 0);
         IO::template store<true>(pl_self, cb, U);
         if (const int edge = slab_edge(a.g, tix)) {          // fused halo push (slab mode only)
             if (edge & 1) IO::template store<true>(IO::plane(a.peer_lo, a.g, mu, p), halo_cb_lo(a.g, cb), U);
