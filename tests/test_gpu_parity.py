@@ -143,7 +143,7 @@ def _thermalised_oracle(O, Nc, n=None):
 
 
 @pytest.mark.parametrize("v", [v for v in VARIANTS if v[1] == "fp64"], ids=_ids)
-@pytest.mark.parametrize("dims", [DIMS_TINY, DIMS_ANISO], ids=["2^4", "4x6x8x10"])
+@pytest.mark.parametrize("dims", [DIMS_TINY, DIMS_ANISO, (2, 6, 4, 8), (6, 2, 8, 2)], ids=["2^4", "4x6x8x10", "2x6x4x8", "6x2x8x2"])
 def test_whole_sweep_fp64(mods, v, dims):
     """P-sweep (north_star: "for a single sweep in fp64, every link element agrees to 1e-11"): su_sweep
     (1 HB + 4 OR = 40 kernels, no re-synchronisation) from the same THERMALISED links. A sweep amplifies

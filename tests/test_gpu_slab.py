@@ -61,6 +61,35 @@ def test_slabs_import_and_halo_push_then_match_the_oracle(mods):
     B.close()
 
 
+def test_thinnest_slabs_and_two_streams(mods):
+    """Lt_local = 2 (every owned slice is both first and last: both halos pushed by every thread), and two
+    independent lattices advancing on two different CUDA streams at once."""
+    import torch
+    su, slab, _ = mods
+    A = su.Lattice(3, DIMS, "fp64")
+    B = slab.SlabGroup(3, DIMS, 4, "fp64")            # 8 time slices -> 4 slabs of 2
+    A.init_hot(2)
+    B.init_hot(2)
+    A.sweep(6.0, 1, 1)
+    B.sweep(6.0, 1, 1)
+    assert np.array_equal(A.export_links(), B.export_links())
+    B.close()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s1):
+        X = su.Lattice(3, DIMS, "fp64")
+    with torch.cuda.stream(s2):
+        Y = su.Lattice(3, DIMS, "fp64")
+    X.init_hot(2)
+    Y.init_hot(2)
+    for _ in range(3):
+        X.sweep(6.0, 1, 1)
+        Y.sweep(6.0, 1, 1)
+    A.sweep(6.0, 1, 1)
+    A.sweep(6.0, 1, 1)
+    ref = A.export_links()
+    assert np.array_equal(X.export_links(), ref) and np.array_equal(Y.export_links(), ref)
+
+
 def test_slab_argument_checks(mods):
     su, slab, _ = mods
     with pytest.raises(ValueError):
