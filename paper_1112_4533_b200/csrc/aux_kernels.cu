@@ -18,17 +18,27 @@ namespace sug {
 // Plaquette (eq 4): per site the six P_mu,nu; Re Tr P = Re Tr[(U_mu(x) U_nu(x+mu))
 // (U_nu(x) U_mu(x+nu))^dagger]. Products in T, site sum and reduction in double.
 // ------------------------------------------------------------------------------------------
+#ifndef SUG_PLAQ_BOTH_PARITIES
+#define SUG_PLAQ_BOTH_PARITIES 1
+#endif
 // Thread -> site: blocks alternate between the two parities of the same lattice region and walk it in the
 // update kernel's z-chunked order (site_of_thread), so a link is fetched from DRAM once: it is read as
 // "own" link by its site and as forward neighbour by three sites of the other parity in the same or the
 // next chunk, all while it is still in L2.
 template <int NC, class T, int STORE, bool UNR>
-__global__ void __launch_bounds__(PLAQ_BLOCK, PLAQ_MINB) k_plaquette(const AuxArgs a) {
+__global__ void __launch_bounds__(PLAQ_BLOCK, (sizeof(T) == 8 ? PLAQ_MINB_F64 : PLAQ_MINB_F32)) k_plaquette(const AuxArgs a) {
     typedef LinkIO<NC, T, STORE, UNR> IO;
     typedef Mat<NC, T, UNR> M;
     typedef cx<T> C;
+#if SUG_PLAQ_BOTH_PARITIES
+    // one block = both parities of PLAQ_BLOCK / 2 consecutive sites: a site's forward neighbours in x and y are own
+    // links of the other half of the block, so they are found in L1
+    const int p = (int)(threadIdx.x / (PLAQ_BLOCK / 2));
+    const unsigned tix = blockIdx.x * (PLAQ_BLOCK / 2) + (threadIdx.x % (PLAQ_BLOCK / 2));
+#else
     const int p = (int)(blockIdx.x & 1u);
     const unsigned tix = (blockIdx.x >> 1) * PLAQ_BLOCK + threadIdx.x;
+#endif
     double acc = 0.0;
     if (tix < a.g.Vh_int) {
         SiteNbr s;
