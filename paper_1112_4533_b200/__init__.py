@@ -14,7 +14,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsugauge.so")
+# SU_GAUGE_LIB selects an ablation build (python -m paper_1112_4533_b200.build with SUG_BUILD_VARIANT); default: the product library
+LIB_PATH = os.environ.get("SU_GAUGE_LIB") or os.path.join(_HERE, "libsugauge.so")
 
 SU_OK, SU_EINVAL, SU_EUNSUPPORTED, SU_ENOMEM, SU_ECUDA, SU_ESTATE = range(6)
 _STATUS = {0: "SU_OK", 1: "SU_EINVAL", 2: "SU_EUNSUPPORTED", 3: "SU_ENOMEM", 4: "SU_ECUDA", 5: "SU_ESTATE"}

@@ -10,8 +10,12 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-OBJ = os.path.join(CSRC, "build")
-LIB = os.path.join(HERE, "libsugauge.so")
+# SUG_BUILD_VARIANT=<name> with SUG_NVCC_EXTRA="-D..." builds libsugauge_<name>.so next to the product library
+# (tuning / ablation builds, e.g. -DSUG_LINK_TILE=1); the product build uses neither.
+VARIANT = os.environ.get("SUG_BUILD_VARIANT", "")
+EXTRA = os.environ.get("SUG_NVCC_EXTRA", "").split() if VARIANT else []
+OBJ = os.path.join(CSRC, "build" + ("_" + VARIANT if VARIANT else ""))
+LIB = os.path.join(HERE, "libsugauge" + ("_" + VARIANT if VARIANT else "") + ".so")
 NCS = list(range(2, 9))
 
 NVCC_FLAGS = [
@@ -40,7 +44,7 @@ def _compile(unit, force, verbose):
     if (not force and os.path.exists(obj)
             and os.path.getmtime(obj) >= max(os.path.getmtime(srcp), _newest_header())):
         return obj, ""
-    cmd = ["nvcc", *NVCC_FLAGS, "-c", srcp, "-o", obj]
+    cmd = ["nvcc", *NVCC_FLAGS, *EXTRA, "-c", srcp, "-o", obj]
     if nc:
         cmd.append(f"-DSUG_NC={nc}")
     if verbose:

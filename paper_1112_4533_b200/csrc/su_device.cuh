@@ -42,7 +42,12 @@ template <class T> __device__ __forceinline__ void mad_ca(cx<T>& acc, cx<T> a, c
 // ------------------------------------------------------------------------------------------
 // Geometry (readings R7): even extents, periodic, checkerboard index cb = i/2.
 // ------------------------------------------------------------------------------------------
-constexpr int LINK_TILE = 32;   // sites per AoSoA tile of the link storage (one warp-wide row per matrix element)
+// sites per AoSoA tile of the link storage (32 = one warp-wide row per matrix element). Overridable for the layout
+// ablation (profiles/r01f): 1 = array of structures, large = structure of arrays.
+#ifndef SUG_LINK_TILE
+#define SUG_LINK_TILE 32
+#endif
+constexpr int LINK_TILE = SUG_LINK_TILE;
 
 struct Geom {
     int L[4];       // extents of the STORED lattice; L[3] includes the two halo time slices in slab mode
