@@ -37,7 +37,7 @@ typedef struct su_lattice su_lattice; /* opaque, owned by the library */
 typedef enum {
     SU_OK = 0,
     SU_EINVAL = 1,       /* NULL pointer, odd or <2 extent, Nc<2, bad beta/pass counts/sizes, RECON12 with Nc!=3 */
-    SU_EUNSUPPORTED = 2, /* Nc above the generic kernel's limit (SU_MAX_NC) */
+    SU_EUNSUPPORTED = 2, /* Nc above the generic kernel's limit (SU_MAX_NC); V >= 2^30 sites (32-bit link indices) */
     SU_ENOMEM = 3,       /* host or device allocation failed / caller buffer too small */
     SU_ECUDA = 4,        /* CUDA error (sticky; text via su_last_error) */
     SU_ESTATE = 5        /* sweep / measurement / export before init or import */
@@ -115,12 +115,14 @@ su_status su_get_counters(su_lattice*, uint64_t* kp_attempts_total, uint64_t* kp
 /* Stream synchronise (surfaces asynchronous errors). */
 su_status su_synchronize(su_lattice*);
 /* Per-handle toggle: capture each distinct (beta, n_hb, n_or) sweep into a CUDA graph and replay it
- * (launch-bound small lattices). Default off. */
+ * (launch-bound small lattices). Default off. At most 16 graphs are cached per handle; a new seed
+ * (su_init_*, su_set_rng) or new peers drop them. SU_EUNSUPPORTED while su_set_timing is on. */
 su_status su_set_graph_mode(su_lattice*, int enabled);
 /* Per-kind device timing of su_sweep (for the benchmark's roofline): when enabled (and graph mode
  * is off) su_sweep records CUDA events on the handle's stream before the heatbath passes, between
  * the heatbath and overrelaxation passes, and after; su_get_timing synchronises and returns the
- * accumulated milliseconds and update-kernel launches per kind since su_set_timing. */
+ * accumulated milliseconds and update-kernel launches per kind since su_set_timing.
+ * SU_EUNSUPPORTED in graph mode (events cannot be read back from a replayed graph). */
 su_status su_set_timing(su_lattice*, int enabled);
 su_status su_get_timing(su_lattice*, double* hb_ms, uint64_t* hb_launches, double* or_ms, uint64_t* or_launches);
 /* Number of kernels this handle has launched so far (for the benchmark's gpu_launches). */
@@ -140,7 +142,8 @@ su_status su_get_launch_count(su_lattice*, uint64_t* out);
  *     su_sweep therefore returns SU_ESTATE on one slab of several; drive su_substep. Sub-step (p, mu) never
  *     reads the halo plane (mu, p), which is the only one its neighbours write meanwhile.
  *   - su_init_cold / su_init_hot / su_reunitarize fill or transform the halos consistently by themselves;
- *     after su_import_links every slab must call su_slab_halo_push once all slabs have imported.
+ *     after su_import_links every slab must call su_slab_halo_push once all slabs have imported; until it
+ *     has, su_sweep / su_substep / su_plaquette / su_reunitarize on that slab return SU_ESTATE.
  *   - su_plaquette returns this slab's SHARE (sum over slabs = the plaquette); su_polyakov and the
  *     attempt-count output of su_substep are SU_EUNSUPPORTED; import / export move the owned slices,
  *     n_doubles = 4 * Lx Ly Lz Lt_local * 2 Nc^2.
@@ -156,6 +159,22 @@ su_status su_slab_halo_push(su_lattice*);
 su_status su_ipc_export(su_lattice*, unsigned char handle[64]);
 su_status su_ipc_open(su_lattice*, const unsigned char handle[64], void** device_ptr);
 su_status su_ipc_close(su_lattice*, void* device_ptr);
+
+/* Sum of the slabs' plaquette shares, for slabs driven by one process (synchronises every slab's stream). */
+su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* out);
+
+/* ---- tuning knobs (none changes a result bit; DESIGN.md names the measured defaults) ----
+ *   "z_chunk_planes"  z-planes per chunk of the update / plaquette kernels' traversal order (a divisor of Lz;
+ *                     0 = the default rule: the largest chunk under 16 MB per time slice). Synchronises.
+ * Unknown names: SU_EINVAL. */
+su_status su_set_option(su_lattice*, const char* name, long long value);
+su_status su_get_option(su_lattice*, const char* name, long long* value);
+
+/* Measured FMA rate of the device's FP32 / FP64 pipes in TFLOP/s (FMA = 2 flops): a short register-only
+ * micro-benchmark (16 independent chains per thread, 8 blocks of 256 threads per SM, best of 5 launches of a few
+ * ms each), the denominator of the "alu" roofline of the variants that are not HBM-bound.
+ * device -1 = current. ms (may be NULL): duration of the best launch. Synchronises the device. */
+su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double* ms);
 
 /* Text of the last error on this handle ("" if none); static text if the handle is NULL.
  * Owned by the library, valid until the next call on the handle. */

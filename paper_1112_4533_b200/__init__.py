@@ -31,7 +31,8 @@ ABI_SYMBOLS = (
     "su_export_links", "su_import_links", "su_set_rng", "su_substep", "su_get_counters",
     "su_synchronize", "su_set_graph_mode", "su_set_timing", "su_get_timing", "su_get_launch_count", "su_last_error",
     "su_lattice_create_slab", "su_slab_bytes", "su_slab_links", "su_slab_set_peers", "su_slab_halo_push",
-    "su_ipc_export", "su_ipc_open", "su_ipc_close",
+    "su_ipc_export", "su_ipc_open", "su_ipc_close", "su_slab_plaquette_sum", "su_set_option", "su_get_option",
+    "su_measure_fma_peak",
 )
 
 
@@ -91,6 +92,10 @@ def lib():
     L.su_ipc_export.argtypes = [P, C.c_char_p]
     L.su_ipc_open.argtypes = [P, C.c_char_p, C.POINTER(P)]
     L.su_ipc_close.argtypes = [P, P]
+    L.su_slab_plaquette_sum.argtypes = [C.POINTER(P), I, C.POINTER(D)]
+    L.su_measure_fma_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D)]
+    L.su_set_option.argtypes = [P, C.c_char_p, C.c_longlong]
+    L.su_get_option.argtypes = [P, C.c_char_p, C.POINTER(C.c_longlong)]
     for name in ABI_SYMBOLS:
         if name not in ("su_lattice_bytes", "su_slab_bytes", "su_last_error"):
             getattr(L, name).restype = I
@@ -108,6 +113,15 @@ def _prec(precision):
 
 def lattice_bytes(Nc, dims, precision="fp64", recon12=False):
     return lib().su_lattice_bytes(Nc, *dims, _prec(precision), SU_STORE_RECON12 if recon12 else SU_STORE_FULL)
+
+
+def measure_fma_peak(precision="fp64", device=-1):
+    """-> (TFLOP/s, ms of the best launch) of the device's FP32 / FP64 FMA pipe (su_measure_fma_peak)"""
+    t, ms = C.c_double(), C.c_double()
+    st = lib().su_measure_fma_peak(device, _prec(precision), C.byref(t), C.byref(ms))
+    if st != SU_OK:
+        raise SuError(st, "su_measure_fma_peak")
+    return t.value, ms.value
 
 
 class Lattice:
@@ -274,6 +288,14 @@ class Lattice:
 
     def ipc_close(self, ptr):
         self._ck(lib().su_ipc_close(self._h, C.c_void_p(ptr)), "su_ipc_close")
+
+    def set_option(self, name, value):
+        self._ck(lib().su_set_option(self._h, name.encode(), int(value)), "su_set_option")
+
+    def get_option(self, name):
+        v = C.c_longlong()
+        self._ck(lib().su_get_option(self._h, name.encode(), C.byref(v)), "su_get_option")
+        return v.value
 
     def launch_count(self):
         n = C.c_uint64()

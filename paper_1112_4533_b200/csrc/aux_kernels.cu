@@ -489,7 +489,7 @@ __global__ void __launch_bounds__(128) k_init_hot(const AuxArgs a) {
 #pragma unroll 1
     for (int b = 0; b < NB; ++b) {
         uint32_t w[4];
-        philox4x32_10(site, 0u, pack_c2(RNG_HOT, 0, p, mu, 0), (uint32_t)b, a.k0, a.k1, w);
+        philox4x32_10(site, 0u, c2_kind(pack_c2(0, p, mu, 0), RNG_HOT), (uint32_t)b, a.k0, a.k1, w);
         for (int h = 0; h < 2; ++h) {
             double ua = uniform01<double>(w[2 * h]), ub = uniform01<double>(w[2 * h + 1]);
             double rad = ::sqrt(-2.0 * ::log(ua));

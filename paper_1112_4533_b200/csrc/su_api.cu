@@ -27,13 +27,17 @@ struct su_lattice {
     void* peer_hi = nullptr;
     bool owns_links = false;
     size_t links_bytes = 0;
+    size_t link_bytes = 0;         // bytes of one stored link
     double* d_partials = nullptr;
     double* d_result = nullptr;
     unsigned long long* d_counters = nullptr;
     uint32_t* d_sweep = nullptr;
     uint8_t* d_attempts = nullptr;
-    double* d_staging = nullptr;
+    double* d_staging[2] = {nullptr, nullptr};   // import / export staging, double-buffered against the PCIe copies
     size_t staging_bytes = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_filled[2] = {nullptr, nullptr}, ev_drained[2] = {nullptr, nullptr};
+    bool halos_valid = true;                     // slab mode: false between su_import_links and su_slab_halo_push
     uint64_t seed = 0;
     uint32_t sweep = 0;
     bool ready = false;
@@ -87,6 +91,9 @@ bool dims_ok(int Nc, int Lx, int Ly, int Lz, int Lt) {
     if (Nc < 2) return false;
     return (double)Lx * Ly * Lz * Lt <= 4294967295.0;   // the site index is one 32-bit RNG counter word
 }
+// The kernels index links (8 V/2 of them) and checkerboard offsets in 32 bits: V < 2^30 keeps every such product
+// in range (176^4 = 0.96e9 sites; SU(2) fp32 at that size is 61 GB). Larger lattices: SU_EUNSUPPORTED.
+bool size_supported(int Lx, int Ly, int Lz, int Lt) { return (double)Lx * Ly * Lz * Lt <= 1073741824.0 - 1024.0; }
 
 int elems_per_link(int Nc, su_storage s) { return Nc == 2 ? 2 : (s == SU_STORE_RECON12 ? 6 : Nc * Nc); }
 // sites stored per (mu, parity) plane: V/2 rounded up to whole tiles of LINK_TILE sites
@@ -126,12 +133,33 @@ int traversal_z_chunk(const Geom& g, size_t link_bytes) {
 AuxArgs aux_args(su_lattice* h) {
     AuxArgs a{};
     a.links = h->links; a.g = h->g; a.partials = h->d_partials; a.result = h->d_result;
-    a.staging = h->d_staging; a.site0 = 0; a.nsites = 0;
+    a.staging = h->d_staging[0]; a.site0 = 0; a.nsites = 0;
     a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
     return a;
 }
 
 __global__ void k_set_u32(uint32_t* p, uint32_t v) { *p = v; }
+
+// FMA-rate micro-benchmark (su_measure_fma_peak): 16 independent accumulator chains per thread, so the pipe is
+// never latency-bound; the operands come from memory so nothing folds at compile time.
+template <class T>
+__global__ void __launch_bounds__(256) k_fma_peak(T* out, const T* in, int iters) {
+    T a[16];
+    const T x = in[0], y = in[1];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = in[2] + (T)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) a[i] = a[i] * x + y;
+        }
+    }
+    T s = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    if (s == (T)123456789) out[blockIdx.x * blockDim.x + threadIdx.x] = s;     // never true: keeps the chains alive
+}
 
 su_status launch_substep(su_lattice* h, double beta, int kind, int pass, int parity, int mu,
                          uint8_t* d_attempts, const uint32_t* d_sweep) {
@@ -195,10 +223,26 @@ su_status enqueue_sweep(su_lattice* h, double beta, int n_hb, int n_or, const ui
     return SU_OK;
 }
 
+// slab mode: after su_import_links the halo slices are stale until every slab has called su_slab_halo_push
+su_status halos_ok(su_lattice* h, const char* who) {
+    if (h->g.t_halo && !h->halos_valid) return fail(h, SU_ESTATE, "%s after su_import_links on a slab: su_slab_halo_push first", who);
+    return SU_OK;
+}
+
 su_status ensure_staging(su_lattice* h, size_t bytes) {
+    if (!h->copy_stream) {
+        SU_CUDA(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking), "copy stream");
+        for (int b = 0; b < 2; ++b) {
+            SU_CUDA(h, cudaEventCreateWithFlags(&h->ev_filled[b], cudaEventDisableTiming), "staging event");
+            SU_CUDA(h, cudaEventCreateWithFlags(&h->ev_drained[b], cudaEventDisableTiming), "staging event");
+        }
+    }
     if (h->staging_bytes >= bytes) return SU_OK;
-    if (h->d_staging) { cudaFree(h->d_staging); h->d_staging = nullptr; h->staging_bytes = 0; }
-    if (cudaMalloc(&h->d_staging, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, SU_ENOMEM, "device staging allocation failed"); }
+    for (int b = 0; b < 2; ++b) {
+        if (h->d_staging[b]) { cudaFree(h->d_staging[b]); h->d_staging[b] = nullptr; }
+        h->staging_bytes = 0;
+        if (cudaMalloc(&h->d_staging[b], bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, SU_ENOMEM, "device staging allocation failed"); }
+    }
     h->staging_bytes = bytes;
     return SU_OK;
 }
@@ -213,7 +257,7 @@ void free_graphs(su_lattice* h) {
 extern "C" {
 
 size_t su_lattice_bytes(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, su_storage s) {
-    if (!dims_ok(Nc, Lx, Ly, Lz, Lt) || (p != SU_FP32 && p != SU_FP64)) return 0;
+    if (!dims_ok(Nc, Lx, Ly, Lz, Lt) || !size_supported(Lx, Ly, Lz, Lt) || (p != SU_FP32 && p != SU_FP64)) return 0;
     if (s != SU_STORE_FULL && s != SU_STORE_RECON12) return 0;
     if (s == SU_STORE_RECON12 && Nc != 3) return 0;
     const size_t Vhp = plane_sites((size_t)Lx * Ly * Lz * Lt / 2);
@@ -238,6 +282,7 @@ static su_status create_common(int Nc, int Lx, int Ly, int Lz, int Lt_glob, bool
     if (o.storage == SU_STORE_RECON12 && Nc != 3) return SU_EINVAL;
     if (o.kernel != SU_KERNEL_AUTO && o.kernel != SU_KERNEL_SPECIALISED && o.kernel != SU_KERNEL_GENERIC) return SU_EINVAL;
     if (Nc > SU_MAX_NC) return SU_EUNSUPPORTED;
+    if (!size_supported(Lx, Ly, Lz, slab ? Lt_loc + 2 : Lt_glob)) return SU_EUNSUPPORTED;
     if (o.kernel == SU_KERNEL_SPECIALISED && Nc > 4) return SU_EUNSUPPORTED;
     if (slab) {
         // whole 32-site tiles per time slice and parity, so that a halo slice of a plane is one contiguous range
@@ -262,7 +307,8 @@ static su_status create_common(int Nc, int Lx, int Ly, int Lz, int Lt_glob, bool
     h->g.Vh = (unsigned)(Vstore / 2);
     h->g.Vhp = (unsigned)plane_sites(Vstore / 2);
     h->var.store = Nc == 2 ? STORE_QUAT : (o.storage == SU_STORE_RECON12 ? STORE_RECON12 : STORE_FULL);
-    h->g.Zc = traversal_z_chunk(h->g, (size_t)elems_per_link(Nc, o.storage) * 2 * (p == SU_FP64 ? 8 : 4));
+    h->link_bytes = (size_t)elems_per_link(Nc, o.storage) * 2 * (p == SU_FP64 ? 8 : 4);
+    h->g.Zc = traversal_z_chunk(h->g, h->link_bytes);
     h->prec = p;
     h->var.Nc = Nc; h->var.prec = (int)p;
     h->var.generic = (o.kernel == SU_KERNEL_GENERIC) || (o.kernel == SU_KERNEL_AUTO && Nc > 4);
@@ -345,6 +391,7 @@ su_status su_slab_halo_push(su_lattice* h) {
         // last owned slice (stored t = Lt_int) -> lower halo of the slab above (their stored t = 0)
         SU_CUDA(h, cudaMemcpyAsync(hi, own + (size_t)h->g.Lt_int * slice, slice, cudaMemcpyDefault, h->stream), "halo push");
     }
+    h->halos_valid = true;
     return SU_OK;
 }
 
@@ -390,7 +437,12 @@ su_status su_lattice_destroy(su_lattice* h) {
     if (h->d_counters) cudaFree(h->d_counters);
     if (h->d_sweep) cudaFree(h->d_sweep);
     if (h->d_attempts) cudaFree(h->d_attempts);
-    if (h->d_staging) cudaFree(h->d_staging);
+    for (int b = 0; b < 2; ++b) {
+        if (h->d_staging[b]) cudaFree(h->d_staging[b]);
+        if (h->ev_filled[b]) cudaEventDestroy(h->ev_filled[b]);
+        if (h->ev_drained[b]) cudaEventDestroy(h->ev_drained[b]);
+    }
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     cudaGetLastError();
     delete h;
     return SU_OK;
@@ -399,7 +451,8 @@ su_status su_lattice_destroy(su_lattice* h) {
 static su_status init_common(su_lattice* h, uint64_t seed, bool hot) {
     if (!h) return SU_EINVAL;
     DeviceGuard guard(h->device);
-    h->seed = seed; h->sweep = 0;
+    if (seed != h->seed) free_graphs(h);             // the Philox key is baked into captured launches
+    h->seed = seed; h->sweep = 0; h->halos_valid = true;
     SU_CUDA(h, cudaMemsetAsync(h->d_counters, 0, 2 * sizeof(unsigned long long), h->stream), "counter reset");
     AuxArgs a = aux_args(h);
     if (hot) SU_CUDA(h, SU_BY_NC(h, init_hot_nc, h->var, a, h->stream, &h->n_launch), "hot start");
@@ -424,6 +477,8 @@ su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
     if (!h->ready) return fail(h, SU_ESTATE, "su_sweep before su_init_* / su_import_links");
     if (h->g.t_halo && !(h->peer_lo == h->links && h->peer_hi == h->links))
         return fail(h, SU_ESTATE, "su_sweep on one slab of several: drive su_substep on all slabs, one sub-step at a time");
+    if (su_status hs = halos_ok(h, "su_sweep")) return hs;
+    if (h->graph_mode && h->timing) return fail(h, SU_EUNSUPPORTED, "su_sweep: per-kind timing is not available in graph mode");
     DeviceGuard guard(h->device);
     if (!h->graph_mode) {
         su_status st = enqueue_sweep(h, beta, n_hb, n_or, nullptr, h->timing);
@@ -433,6 +488,7 @@ su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
         auto key = std::make_tuple(beta, n_hb, n_or);
         auto it = h->graphs.find(key);
         if (it == h->graphs.end()) {
+            if (h->graphs.size() >= 16) free_graphs(h);      // e.g. annealing over many beta: bound the cache
             cudaStream_t cap;
             SU_CUDA(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking), "graph capture stream");
             cudaStream_t user = h->stream;
@@ -469,6 +525,7 @@ su_status su_substep(su_lattice* h, double beta, int kind, int pass, int parity,
         return fail(h, SU_EINVAL, "su_substep: argument out of range");
     if (!h->ready) return fail(h, SU_ESTATE, "su_substep before su_init_* / su_import_links");
     if (host_attempts && h->g.t_halo) return fail(h, SU_EUNSUPPORTED, "attempt counts are not exported in slab mode");
+    if (su_status hs = halos_ok(h, "su_substep")) return hs;
     DeviceGuard guard(h->device);
     const size_t nsub = (size_t)h->Nc * (h->Nc - 1) / 2, nbytes = nsub * h->g.Vh;
     if (host_attempts) {
@@ -490,6 +547,7 @@ su_status su_substep(su_lattice* h, double beta, int kind, int pass, int parity,
 su_status su_plaquette(su_lattice* h, double* out) {
     if (!h || !out) return SU_EINVAL;
     if (!h->ready) return fail(h, SU_ESTATE, "su_plaquette before su_init_* / su_import_links");
+    if (su_status hs = halos_ok(h, "su_plaquette")) return hs;
     DeviceGuard guard(h->device);
     AuxArgs a = aux_args(h);
     SU_CUDA(h, SU_BY_NC(h, plaquette_nc, h->var, a, h->stream, &h->n_launch), "plaquette kernels");
@@ -517,34 +575,49 @@ su_status su_polyakov(su_lattice* h, double out[2]) {
 su_status su_reunitarize(su_lattice* h) {
     if (!h) return SU_EINVAL;
     if (!h->ready) return fail(h, SU_ESTATE, "su_reunitarize before su_init_* / su_import_links");
+    if (su_status hs = halos_ok(h, "su_reunitarize")) return hs;
     DeviceGuard guard(h->device);
     AuxArgs a = aux_args(h);
     SU_CUDA(h, SU_BY_NC(h, reunit_nc, h->var, a, h->stream, &h->n_launch), "reunitarise kernel");
     return SU_OK;
 }
 
+// Layout conversion runs on the lattice's stream, the PCIe copy on a second stream; two staging buffers, so the
+// conversion kernel of chunk i+1 overlaps the copy of chunk i (events order the hand-over in both directions).
 static su_status transfer_links(su_lattice* h, double* host, size_t n_doubles, bool to_host) {
     const size_t per_site = 4 * 2 * (size_t)h->Nc * h->Nc;                  // doubles per site
     if (n_doubles != h->V * per_site) return fail(h, SU_EINVAL, "link array size must be 4 V * 2 Nc^2 doubles");
     DeviceGuard guard(h->device);
-    const size_t chunk_sites_max = (size_t)(64u << 20) / (per_site * sizeof(double)) + 1;
+    const size_t chunk_sites_max = (size_t)(32u << 20) / (per_site * sizeof(double)) + 1;
     const size_t chunk_sites = chunk_sites_max < h->V ? chunk_sites_max : h->V;
     su_status st = ensure_staging(h, chunk_sites * per_site * sizeof(double));
     if (st != SU_OK) return st;
-    for (size_t s0 = 0; s0 < h->V; s0 += chunk_sites) {
+    int i = 0;
+    for (size_t s0 = 0; s0 < h->V; s0 += chunk_sites, ++i) {
+        const int b = i & 1;
         const size_t ns = (h->V - s0 < chunk_sites) ? h->V - s0 : chunk_sites;
         AuxArgs a = aux_args(h);
+        a.staging = h->d_staging[b];
         a.site0 = (unsigned)s0; a.nsites = (unsigned)ns;
         double* hp = host + s0 * per_site;
         if (to_host) {
+            if (i >= 2) SU_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_drained[b], 0), "export ordering");
             SU_CUDA(h, SU_BY_NC(h, export_nc, h->var, a, h->stream, &h->n_launch), "export kernel");
-            SU_CUDA(h, cudaMemcpyAsync(hp, h->d_staging, ns * per_site * sizeof(double), cudaMemcpyDeviceToHost, h->stream), "export copy");
+            SU_CUDA(h, cudaEventRecord(h->ev_filled[b], h->stream), "export ordering");
+            SU_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->ev_filled[b], 0), "export ordering");
+            SU_CUDA(h, cudaMemcpyAsync(hp, h->d_staging[b], ns * per_site * sizeof(double), cudaMemcpyDeviceToHost, h->copy_stream), "export copy");
+            SU_CUDA(h, cudaEventRecord(h->ev_drained[b], h->copy_stream), "export ordering");
         } else {
-            SU_CUDA(h, cudaMemcpyAsync(h->d_staging, hp, ns * per_site * sizeof(double), cudaMemcpyHostToDevice, h->stream), "import copy");
+            if (i >= 2) SU_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->ev_drained[b], 0), "import ordering");
+            SU_CUDA(h, cudaMemcpyAsync(h->d_staging[b], hp, ns * per_site * sizeof(double), cudaMemcpyHostToDevice, h->copy_stream), "import copy");
+            SU_CUDA(h, cudaEventRecord(h->ev_filled[b], h->copy_stream), "import ordering");
+            SU_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_filled[b], 0), "import ordering");
             SU_CUDA(h, SU_BY_NC(h, import_nc, h->var, a, h->stream, &h->n_launch), "import kernel");
+            SU_CUDA(h, cudaEventRecord(h->ev_drained[b], h->stream), "import ordering");
         }
-        SU_CUDA(h, cudaStreamSynchronize(h->stream), "link transfer synchronise");
     }
+    SU_CUDA(h, cudaStreamSynchronize(h->copy_stream), "link transfer synchronise");
+    SU_CUDA(h, cudaStreamSynchronize(h->stream), "link transfer synchronise");
     return SU_OK;
 }
 
@@ -557,7 +630,7 @@ su_status su_export_links(su_lattice* h, double* host_dst, size_t n_doubles) {
 su_status su_import_links(su_lattice* h, const double* host_src, size_t n_doubles) {
     if (!h || !host_src) return SU_EINVAL;
     su_status st = transfer_links(h, const_cast<double*>(host_src), n_doubles, false);
-    if (st == SU_OK) h->ready = true;
+    if (st == SU_OK) { h->ready = true; if (h->g.t_halo) h->halos_valid = false; }
     return st;
 }
 
@@ -581,12 +654,14 @@ su_status su_synchronize(su_lattice* h) {
 
 su_status su_set_graph_mode(su_lattice* h, int enabled) {
     if (!h) return SU_EINVAL;
+    if (enabled && h->timing) return fail(h, SU_EUNSUPPORTED, "su_set_graph_mode: per-kind timing is on (events cannot be read back from a replayed graph)");
     h->graph_mode = enabled != 0;
     return SU_OK;
 }
 
 su_status su_set_timing(su_lattice* h, int enabled) {
     if (!h) return SU_EINVAL;
+    if (enabled && h->graph_mode) return fail(h, SU_EUNSUPPORTED, "su_set_timing: not available in graph mode");
     DeviceGuard guard(h->device);
     drain_timing(h);
     h->timing = enabled != 0;
@@ -608,6 +683,79 @@ su_status su_get_timing(su_lattice* h, double* hb_ms, uint64_t* hb_launches, dou
 su_status su_get_launch_count(su_lattice* h, uint64_t* out) {
     if (!h || !out) return SU_EINVAL;
     *out = h->n_launch;
+    return SU_OK;
+}
+
+su_status su_set_option(su_lattice* h, const char* name, long long value) {
+    if (!h || !name) return SU_EINVAL;
+    DeviceGuard guard(h->device);
+    if (!strcmp(name, "z_chunk_planes")) {
+        // traversal order of the update / plaquette kernels: planes per z-chunk, a divisor of Lz (0 = the default rule)
+        if (value < 0 || value > h->g.L[2] || (value > 0 && h->g.L[2] % value)) return fail(h, SU_EINVAL, "z_chunk_planes must divide Lz");
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);
+        h->g.Zc = value > 0 ? (int)value : traversal_z_chunk(h->g, h->link_bytes);
+        return SU_OK;
+    }
+    return fail(h, SU_EINVAL, "su_set_option: unknown option '%s'", name);
+}
+
+su_status su_get_option(su_lattice* h, const char* name, long long* value) {
+    if (!h || !name || !value) return SU_EINVAL;
+    if (!strcmp(name, "z_chunk_planes")) { *value = h->g.Zc; return SU_OK; }
+    return fail(h, SU_EINVAL, "su_get_option: unknown option '%s'", name);
+}
+
+su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* out) {
+    if (!slabs || n_slabs < 1 || !out) return SU_EINVAL;
+    double sum = 0;
+    for (int r = 0; r < n_slabs; ++r) {
+        double share = 0;
+        su_status st = su_plaquette(slabs[r], &share);
+        if (st != SU_OK) return st;
+        sum += share;
+    }
+    *out = sum;
+    return SU_OK;
+}
+
+su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double* ms) {
+    if (!tflops || (p != SU_FP32 && p != SU_FP64)) return SU_EINVAL;
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return SU_ECUDA;
+    DeviceGuard guard(dev);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SU_ECUDA;
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = p == SU_FP64 ? 4096 : 16384;
+    void *in = nullptr, *out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    su_status st = SU_OK;
+    const double host_in64[3] = {1.0000001, 1e-9, 0.5};
+    const float host_in32[3] = {1.0000001f, 1e-9f, 0.5f};
+    if (cudaMalloc(&in, 3 * sizeof(double)) != cudaSuccess || cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)) != cudaSuccess ||
+        cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) st = SU_ENOMEM;
+    float best = 0;
+    if (st == SU_OK) {
+        cudaMemcpy(in, p == SU_FP64 ? (const void*)host_in64 : (const void*)host_in32, p == SU_FP64 ? 24 : 12, cudaMemcpyHostToDevice);
+        for (int rep = 0; rep < 6 && st == SU_OK; ++rep) {          // first repetition = warm-up
+            cudaEventRecord(e0, 0);
+            if (p == SU_FP64) k_fma_peak<double><<<blocks, threads>>>((double*)out, (const double*)in, iters);
+            else              k_fma_peak<float><<<blocks, threads>>>((float*)out, (const float*)in, iters);
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { st = SU_ECUDA; break; }
+            float t = 0;
+            cudaEventElapsedTime(&t, e0, e1);
+            if (rep > 0 && (best == 0 || t < best)) best = t;
+        }
+    }
+    if (in) cudaFree(in);
+    if (out) cudaFree(out);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (st != SU_OK) { cudaGetLastError(); return st; }
+    const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;     // 64 FMAs per iteration per thread
+    *tflops = flops / ((double)best * 1e-3) / 1e12;
+    if (ms) *ms = best;
     return SU_OK;
 }
 

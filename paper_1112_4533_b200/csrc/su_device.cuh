@@ -318,10 +318,12 @@ template <class T> __device__ __forceinline__ T uniform01(uint32_t w);
 template <> __device__ __forceinline__ double uniform01<double>(uint32_t w) { return ((double)w + 1.0) * (1.0 / 4294967296.0); }
 template <> __device__ __forceinline__ float  uniform01<float >(uint32_t w) { return ((float)(w >> 8) + 1.0f) * (1.0f / 16777216.0f); }
 
-__device__ __forceinline__ uint32_t pack_c2(int kind, int pass, int parity, int mu, int subgroup) {
-    return ((uint32_t)kind << 28) | ((uint32_t)(pass & 0xff) << 20) | ((uint32_t)parity << 19) |
-           ((uint32_t)mu << 17) | (uint32_t)subgroup;
+// Counter word c2 = kind<<28 | pass<<20 | parity<<19 | mu<<17 | subgroup. pack_c2 fills
+// the low 28 bits; the stream kind (RNG_KP / RNG_DIR / RNG_HOT) is ORed in by c2_kind where a block is drawn.
+__device__ __forceinline__ uint32_t pack_c2(int pass, int parity, int mu, int subgroup) {
+    return ((uint32_t)(pass & 0xff) << 20) | ((uint32_t)parity << 19) | ((uint32_t)mu << 17) | (uint32_t)subgroup;
 }
+__device__ __forceinline__ uint32_t c2_kind(uint32_t c2_low, int kind) { return c2_low | ((uint32_t)kind << 28); }
 
 template <class T> struct Fn;
 template <> struct Fn<float> {
@@ -364,7 +366,7 @@ template <> struct Fn<double> {
 template <class T>
 __device__ __forceinline__ void kp_direction(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2_base, T n[3]) {
     uint32_t d[4];
-    philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_DIR << 28), 0u, k0, k1, d);
+    philox4x32_10(c0, c1, c2_kind(c2_base, RNG_DIR), 0u, k0, k1, d);
     const T u1 = uniform01<T>(d[0]), u2 = uniform01<T>(d[1]);
     const T cos_t = (T)1 - (T)2 * u1;
     const T sin_t = Fn<T>::sqrt(Fn<T>::max0((T)1 - cos_t * cos_t));
@@ -374,9 +376,11 @@ __device__ __forceinline__ void kp_direction(uint32_t k0, uint32_t k1, uint32_t 
 }
 
 template <class T>
-__device__ __forceinline__ int kp_draw(T alpha, T m_inv2a, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
+__device__ __forceinline__ int kp_draw(unsigned draw_mask, T alpha, T m_inv2a, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
                                        uint32_t c2_base, T v[4], const T* dir = nullptr, int dir_stride = 0) {
-    if (!(alpha > (T)0) || !Fn<T>::finite(alpha)) return 0;
+    const bool drawable = (alpha > (T)0) && Fn<T>::finite(alpha);
+    const unsigned converged = __ballot_sync(draw_mask, drawable);
+    if (!drawable) return 0;
     constexpr bool PRETEST = (sizeof(T) == 8) && (SUG_KP_PRETEST != 0);
     const float two_af = 2.0f * (float)alpha;
     const float band = 1e-3f + two_af * 4e-6f;
@@ -385,10 +389,11 @@ __device__ __forceinline__ int kp_draw(T alpha, T m_inv2a, uint32_t k0, uint32_t
     uint32_t w[4];
     // lanes leave the accept loop after different numbers of attempts; without an explicit barrier the
     // compiler lets every exit group run the rest of the draw on its own (ncu: the direction part ran 1.6x
-    // per warp). The mask is the set of lanes converged here, so the barrier is safe in a ragged last warp.
-    const unsigned converged = __activemask();
+    // per warp). draw_mask = the lanes that call kp_draw for this subgroup, balloted by the caller BEFORE its
+    // divergent branch (all of them reach the barrier: the early return above is taken before the loop by
+    // lanes that then skip it, so they are excluded here).
     for (int n = 0; n < KP_MAX_ATTEMPTS; ++n) {
-        philox4x32_10(c0, c1, c2_base | ((uint32_t)RNG_KP << 28), (uint32_t)n, k0, k1, w);
+        philox4x32_10(c0, c1, c2_kind(c2_base, RNG_KP), (uint32_t)n, k0, k1, w);
         if (PRETEST) {
             const float S = 2.3283064365386963e-10f;      // 2^-32
             const float r1f = (__uint2float_rn(w[0]) + 1.0f) * S, r2f = (__uint2float_rn(w[1]) + 1.0f) * S;
@@ -437,8 +442,10 @@ template <int NC, class T, int KIND, bool UNR>
 __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uint32_t k0, uint32_t k1,
                                                  uint32_t c0, uint32_t c1, uint32_t c2_base,
                                                  uint8_t* att_out, size_t att_stride,
-                                                 unsigned& att_total, unsigned& exhausted,
+                                                 unsigned& att_total, unsigned& exhausted, unsigned warp_mask,
                                                  const T* dirs = nullptr, int dir_stride = 0) {
+    // warp_mask: the lanes of this warp that run the subgroup loop (balloted by the kernel where all of them
+    // are converged); every one of them executes the ballots below, subgroup by subgroup
     int q = 0;
     const T two_beta_over_nc = (T)2 * beta / (T)NC;      // alpha = 2 beta k / Nc (reading R3)
     const T m_nc_over_4beta = (T)-0.25 * (T)NC / beta;   // -1 / (2 alpha) = this / k   (heatbath only)
@@ -453,12 +460,13 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
             bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
             T a[4] = {(T)1, (T)0, (T)0, (T)0};
             int used = 0;
+            const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
             if (ok) {
                 if (KIND == KIND_HB) {
                     const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;          // 1/k and k without a division
                     T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                     T v[4];
-                    used = kp_draw<T>(two_beta_over_nc * k, m_nc_over_4beta * ik, k0, k1, c0, c1,
+                    used = kp_draw<T>(draw_mask, two_beta_over_nc * k, m_nc_over_4beta * ik, k0, k1, c0, c1,
                                       c2_base | (uint32_t)q, v, dirs ? dirs + 3 * q * dir_stride : nullptr, dir_stride);
                     if (used) quat_mul(v, ud, a); else ok = false;
                 } else {

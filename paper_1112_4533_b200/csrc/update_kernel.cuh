@@ -100,6 +100,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
     typedef cx<T> C;
     const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = tix < a.g.Vh_int;
+    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);      // lanes that run the body (ragged last warp)
     unsigned att_total = 0, exhausted = 0;
     if (active) {
         const int p = a.parity, mu = a.mu;
@@ -118,7 +119,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
 #pragma unroll
             for (int q = 0; q < NSUB; ++q) {
                 T n[3];
-                kp_direction<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2(0, (int)a.pass, p, mu, q), n);
+                kp_direction<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2((int)a.pass, p, mu, q), n);
                 dir_sm[3 * q][threadIdx.x] = n[0]; dir_sm[3 * q + 1][threadIdx.x] = n[1]; dir_sm[3 * q + 2][threadIdx.x] = n[2];
             }
         }
@@ -173,9 +174,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
         IO::template load<LD_STREAM>(pl_self, cb, U);
         M::mul_nd(U, S, W);                                   // W = U S^dagger
         update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex, sweep_ctr,
-                                           pack_c2(0, (int)a.pass, p, mu, 0),
+                                           pack_c2((int)a.pass, p, mu, 0),
                                            a.attempts ? a.attempts + cb : nullptr, (size_t)a.g.Vh,
-                                           att_total, exhausted,
+                                           att_total, exhausted, warp_mask,
                                            PREDIR ? &dir_sm[0][threadIdx.x] : nullptr, PREDIR ? BLOCK : 0);
         IO::template store<true>(pl_self, cb, U);
         if (const int edge = slab_edge(a.g, tix)) {          // fused halo push (slab mode only)
@@ -216,6 +217,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
     typedef typename V2<T>::type T2;
     const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = tix < a.g.Vh_int;
+    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);
     unsigned att_total = 0, exhausted = 0;
     if (active) {
         const int p = a.parity, mu = a.mu;
@@ -253,13 +255,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
         const T n2 = W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3];      // k^2
         bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
         int used = 0;
+        const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
         if (ok) {
             if (KIND == KIND_HB) {
                 const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;
                 T ud[4] = {W[0] * ik, -W[1] * ik, -W[2] * ik, -W[3] * ik};
                 T v[4];
-                used = kp_draw<T>((T)a.beta * k, (T)-0.5 / (T)a.beta * ik, a.k0, a.k1, s.lex, a.sweep_ptr ? *a.sweep_ptr : a.sweep,
-                                  pack_c2(0, (int)a.pass, p, mu, 0), v);
+                used = kp_draw<T>(draw_mask, (T)a.beta * k, (T)-0.5 / (T)a.beta * ik, a.k0, a.k1, s.lex, a.sweep_ptr ? *a.sweep_ptr : a.sweep,
+                                  pack_c2((int)a.pass, p, mu, 0), v);
                 if (used) quat_mul(v, ud, a4); else ok = false;
             } else {
                 // a = conj(W)^2 / k^2 (eq 17)

@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
     const T two_beta_over_nc = (T)2 * beta / (T)NC;
     const T m_nc_over_4beta = (T)-0.25 * (T)NC / beta;
     const uint32_t c1 = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
-    const uint32_t c2_base = pack_c2(0, (int)a.pass, p, mu, 0);
+    const uint32_t c2_base = pack_c2((int)a.pass, p, mu, 0);
     unsigned att_total = 0, exhausted = 0;
     // Wavefront over the lexicographic subgroup order: step (i,j) only depends on earlier steps that touched
     // row i or row j, and steps on disjoint row pairs commute exactly (A_ij is built from rows i,j of W and
@@ -188,12 +188,13 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
         bool ok = paired && (n2 > (T)0) && Fn<T>::finite(n2);
         T q4[4] = {(T)1, (T)0, (T)0, (T)0};
         int used = 0;
+        const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(0xffffffffu, ok) : 0u;   // all 32 lanes are here
         if (ok) {
             if (KIND == KIND_HB) {
                 const T ik = Fn<T>::rsqrt(n2), kk = n2 * ik;
                 T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                 T v[4];
-                used = kp_draw<T>(two_beta_over_nc * kk, m_nc_over_4beta * ik, a.k0, a.k1, s.lex, c1,
+                used = kp_draw<T>(draw_mask, two_beta_over_nc * kk, m_nc_over_4beta * ik, a.k0, a.k1, s.lex, c1,
                                   c2_base | (uint32_t)sub, v);
                 if (used) quat_mul(v, ud, q4); else ok = false;
             } else {

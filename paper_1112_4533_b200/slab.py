@@ -4,17 +4,21 @@ Argument marshalling and ordering only: the arithmetic, including the halo push,
 (the update kernel stores the links of a slab's first / last owned time slice straight into the neighbour
 slab's halo - peer memory over NVLink when the slabs sit on different GPUs).
 
-  SlabGroup           n slabs driven by ONE process (one device, or several with peer access): used by the
-                      tests to prove that n slabs reproduce the single-lattice chain exactly.
+  SlabGroup           n slabs driven by ONE process on ONE device and one stream: used by the tests to prove
+                      that n slabs reproduce the single-lattice chain exactly.
   DistributedLattice  one slab per torch.distributed rank (one process per GPU): peers through CUDA IPC, the
-                      ordering between sub-steps through a stream-ordered NCCL all-reduce of one element.
+                      ordering between sub-steps through a stream-ordered NCCL all-reduce of one element
+                      (order="nccl"), or through su_synchronize + a host barrier (order="host": any backend,
+                      e.g. gloo when two test ranks share one GPU).
 
 The sweep schedule is the single-lattice one (R6): every sub-step (pass, parity, mu) on all slabs,
 then the next; the handles' sweep counters advance together.
 """
+import ctypes as C
+
 import numpy as np
 
-from . import Lattice
+from . import Lattice, SuError, SU_OK, lib
 
 
 def slab_starts(Lt_global, n_slabs):
@@ -40,14 +44,14 @@ def schedule(n_hb, n_or):
 
 
 class SlabGroup:
-    """A lattice cut into n_slabs t-slabs, all driven from this process on one stream (same-stream order is
-    the ordering the ABI asks for). devices: one CUDA ordinal per slab (default: all on `device`)."""
+    """A lattice cut into n_slabs t-slabs, all on ONE device and driven from this process on one stream
+    (same-stream order is the ordering the ABI asks for). Slabs on several devices need one process per device:
+    DistributedLattice."""
 
-    def __init__(self, Nc, dims, n_slabs, precision="fp64", recon12=False, kernel="auto", device=0, devices=None):
+    def __init__(self, Nc, dims, n_slabs, precision="fp64", recon12=False, kernel="auto", device=0):
         starts, lt = slab_starts(dims[3], n_slabs)
-        devices = devices or [device] * n_slabs
         self.Nc, self.dims, self.n = Nc, tuple(dims), n_slabs
-        self.slabs = [Lattice(Nc, dims, precision, recon12, kernel, device=devices[r], slab=(starts[r], lt))
+        self.slabs = [Lattice(Nc, dims, precision, recon12, kernel, device=device, slab=(starts[r], lt))
                       for r in range(n_slabs)]
         ptrs = [s.links_ptr()[0] for s in self.slabs]
         for r, s in enumerate(self.slabs):
@@ -86,7 +90,12 @@ class SlabGroup:
             s.reunitarize()
 
     def plaquette(self):
-        return sum(s.plaquette() for s in self.slabs)
+        handles = (C.c_void_p * self.n)(*[s._h for s in self.slabs])
+        out = C.c_double()
+        st = lib().su_slab_plaquette_sum(handles, self.n, C.byref(out))
+        if st != SU_OK:
+            raise SuError(st, "su_slab_plaquette_sum")
+        return out.value
 
     def export_links(self):
         return np.concatenate([s.export_links() for s in self.slabs], axis=0)
@@ -104,14 +113,19 @@ class SlabGroup:
 
 
 class DistributedLattice:
-    """One t-slab per rank of an initialised torch.distributed process group (backend nccl, one process per
-    GPU of one node). Neighbours' link buffers are mapped with CUDA IPC; between two sub-steps a one-element
-    all-reduce, enqueued on the lattice's stream, orders the ranks without blocking the host."""
+    """One t-slab per rank of an initialised torch.distributed process group (one process per GPU of one
+    node). Neighbours' link buffers are mapped with CUDA IPC. Ordering between sub-steps (and after every call
+    that rewrites halo slices: init, reunitarise, halo push):
+      order="nccl"  a one-element all-reduce enqueued on the lattice's stream: stream-ordered, the host never blocks;
+      order="host"  su_synchronize + dist.barrier(): works with any backend (gloo), used when NCCL cannot run,
+                    e.g. two test ranks sharing one GPU."""
 
-    def __init__(self, Nc, dims, precision="fp64", recon12=False, kernel="auto", device=None):
+    def __init__(self, Nc, dims, precision="fp64", recon12=False, kernel="auto", device=None, order="nccl"):
         import torch
         import torch.distributed as dist
-        self.dist, self.torch = dist, torch
+        if order not in ("nccl", "host"):
+            raise ValueError("order must be 'nccl' or 'host'")
+        self.dist, self.torch, self.order = dist, torch, order
         self.rank, self.world = dist.get_rank(), dist.get_world_size()
         starts, lt = slab_starts(dims[3], self.world)
         device = torch.cuda.current_device() if device is None else device
@@ -127,13 +141,17 @@ class DistributedLattice:
                 ptr[r] = self.lat.ipc_open(handles[r])
                 self._opened.append(ptr[r])
         self.lat.set_peers(ptr[below], ptr[above])
-        self._token = torch.zeros(1, device=self.lat.device)
+        self._token = torch.zeros(1, device=self.lat.device) if order == "nccl" else None
         self.seed, self.sweep_counter = 0, 0
 
     def _order(self):
-        # stream-ordered: the collective waits for the kernels already enqueued on the current stream
-        # (the lattice's stream) and later kernels on that stream wait for it
-        self.dist.all_reduce(self._token)
+        if self.order == "nccl":
+            # stream-ordered: the collective waits for the kernels already enqueued on the current stream
+            # (the lattice's stream) and later kernels on that stream wait for it
+            self.dist.all_reduce(self._token)
+        else:
+            self.lat.synchronize()
+            self.dist.barrier()
 
     def close(self):
         self._order()
@@ -161,10 +179,14 @@ class DistributedLattice:
         self.lat.set_rng(self.seed, self.sweep_counter)
 
     def reunitarize(self):
+        # su_reunitarize rewrites the halo slices too (consistently: the same links, the same arithmetic); a
+        # neighbour must not start pushing the next sub-step's links into them before that is finished
         self.lat.reunitarize()
+        self._order()
 
     def plaquette(self):
-        t = self.torch.tensor([self.lat.plaquette()], dtype=self.torch.float64, device=self.lat.device)
+        dev = self.lat.device if self.order == "nccl" else "cpu"
+        t = self.torch.tensor([self.lat.plaquette()], dtype=self.torch.float64, device=dev)
         self.dist.all_reduce(t)
         return float(t.item())
 

@@ -1,0 +1,112 @@
+"""DistributedLattice (paper_1112_4533_b200/slab.py) on the one GPU the
+tests have (pytest -m gpu):
+  * world_size 1 over NCCL: one self-peered slab in a library-owned buffer, CUDA IPC export, the stream-ordered
+    all-reduce between sub-steps - bitwise the plain Lattice;
+  * TWO processes sharing cuda:0 (tests/dist_worker.py): the neighbours' buffers are opened through CUDA IPC and the
+    update kernels push their boundary links into them; ordering by su_synchronize + a gloo barrier. Bitwise the
+    single lattice, and 1e-11 from the oracle's next sweep."""
+import os
+import socket
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+DIMS = (8, 4, 8, 8)
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def mods():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import oracle
+    import paper_1112_4533_b200 as su
+    return su, oracle
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def test_world_size_one_over_nccl_is_the_plain_lattice(mods):
+    import torch
+    import torch.distributed as dist
+    su, _ = mods
+    from paper_1112_4533_b200.slab import DistributedLattice
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{_free_port()}", rank=0, world_size=1,
+                            device_id=torch.device("cuda", 0))
+    try:
+        for Nc, precision, recon12, beta in [(3, "fp64", False, 6.0), (2, "fp32", False, 2.3), (6, "fp64", False, 25.0)]:
+            A = su.Lattice(Nc, DIMS, precision, recon12)
+            D = DistributedLattice(Nc, DIMS, precision, recon12, device=0)
+            assert len(D.lat.ipc_export()) == 64
+            A.init_hot(4)
+            D.init_hot(4)
+            for _ in range(2):
+                A.sweep(beta, 1, 2)
+                D.sweep(beta, 1, 2)
+                A.reunitarize()
+                D.reunitarize()
+            assert np.array_equal(A.export_links(), D.export_links())
+            assert abs(A.plaquette() - D.plaquette()) < 1e-14
+            snap = A.export_links()
+            D.import_links(snap)                    # import -> halo push -> next sweep
+            A.sweep(beta, 1, 1)
+            D.sweep(beta, 1, 1)
+            assert np.array_equal(A.export_links(), D.export_links())
+            D.close()
+            A.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("Nc,precision,recon12,kernel,beta", [
+    (3, "fp64", False, "auto", 6.0), (3, "fp32", True, "auto", 6.0), (2, "fp64", False, "auto", 2.3),
+    (4, "fp64", False, "generic", 11.0)], ids=["su3-fp64", "su3-fp32-r12", "su2-fp64", "su4-generic"])
+def test_two_processes_one_gpu_ipc_and_peer_halo_push(mods, tmp_path, Nc, precision, recon12, kernel, beta):
+    su, oracle = mods
+    O = oracle.OracleLattice(Nc, DIMS, precision, recon12)
+    O.init_hot(9)
+    for _ in range(3):
+        O.sweep(beta, 1, 4)
+    start = O.export_links()
+    np.save(tmp_path / "start.npy", start)
+    np.save(tmp_path / "cfg.npy", dict(Nc=Nc, dims=DIMS, precision=precision, recon12=recon12, kernel=kernel,
+                                       beta=beta, seed=9, sweep0=3), allow_pickle=True)
+    port = str(_free_port())
+    procs = [subprocess.Popen([sys.executable, os.path.join(HERE, "dist_worker.py"), str(r), "2", port, str(tmp_path)],
+                              stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for r in range(2)]
+    outs = []
+    for p in procs:
+        try:
+            outs.append(p.communicate(timeout=600)[0])
+        except subprocess.TimeoutExpired:
+            for q in procs:
+                q.kill()
+            raise
+    assert all(p.returncode == 0 for p in procs), "\n".join(outs)
+    after1 = np.concatenate([np.load(tmp_path / f"after1_{r}.npy") for r in range(2)], axis=0)
+    after2 = np.concatenate([np.load(tmp_path / f"after2_{r}.npy") for r in range(2)], axis=0)
+    # the single lattice, same inputs
+    A = su.Lattice(Nc, DIMS, precision, recon12, kernel)
+    A.import_links(start)
+    A.set_rng(9, 3)
+    A.sweep(beta, 1, 4)
+    assert np.array_equal(A.export_links(), after1)
+    assert abs(A.plaquette() - float(np.load(tmp_path / "plaq.npy")[0])) < 1e-13
+    if precision == "fp64":
+        O.sweep(beta, 1, 4)
+        assert np.abs(after1 - O.export_links()).max() <= 1e-11
+    A.reunitarize()
+    A.sweep(beta, 1, 2)
+    A.reunitarize()
+    A.sweep(beta, 0, 1)
+    assert np.array_equal(A.export_links(), after2)

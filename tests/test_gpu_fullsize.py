@@ -169,3 +169,69 @@ def test_thermalised_means_agree_statistically(mods, Nc, L, beta):
     (mg, eg), (mo, eo) = mean_err(pg), mean_err(po)
     assert abs(mg - mo) <= 3.0 * np.hypot(eg, eo), (mg, eg, mo, eo)
     assert G.counters()[1] == 0
+
+
+def test_su3_48_whole_sweep_every_link(mods):
+    """P-sweep at full size: one whole su_sweep(1, 4) = 40 kernels at 48^4 fp64 (the z-chunked traversal, the
+    launch configuration bench.py times) against the oracle's sweep, all 21 M links at 1e-11, from links the
+    ORACLE has thermalised (3 sweeps of 1 HB + 4 OR from the hot start, ~10 s each on the box's cores)."""
+    su, oracle = mods
+    dims = (L_FULL,) * 4
+    O = oracle.OracleLattice(3, dims, "fp64")
+    O.init_hot(SEED)
+    for _ in range(3):
+        O.sweep(BETA, 1, 4)
+    G = su.Lattice(3, dims, "fp64")
+    assert G.get_option("z_chunk_planes") < L_FULL          # the chunked traversal is what runs here
+    G.import_links(O.export_links())
+    G.set_rng(SEED, 3)
+    att0 = O.counters()[0]
+    G.sweep(BETA, 1, 4)
+    O.sweep(BETA, 1, 4)
+    lg, lo = G.export_links(), O.export_links()
+    assert _maxdiff(lg, lo) <= 1e-11
+    assert G.counters()[0] == O.counters()[0] - att0 and G.counters()[1] == 0
+    assert abs(G.plaquette() - O.plaquette()) < 1e-12
+    assert abs(G.polyakov() - O.polyakov()) < 1e-12
+
+
+@pytest.mark.parametrize("Nc,L,beta,seed,start,precision,kernel", [
+    (4, 24, 11.0, 11, "hot", "fp64", "auto"), (4, 24, 11.0, 11, "hot", "fp32", "auto"),
+    (4, 24, 11.0, 11, "hot", "fp64", "generic"), (6, 16, 25.0, 5, "cold", "fp64", "auto")],
+    ids=["su4-24-fp64", "su4-24-fp32", "su4-24-fp64-generic", "su6-16-fp64"])
+def test_config4_and_config5_lockstep_at_their_own_size(mods, Nc, L, beta, seed, start, precision, kernel):
+    """BASELINE.json configs[3] (SU(4) 24^4, specialised and generic kernel) and configs[4] (SU(6) 16^4) at their
+    own sizes: heatbath and overrelaxation sub-steps in lock-step with the oracle on links the oracle has ordered
+    with one 1 HB + 1 OR sweep; every link, attempt counts per (link, subgroup)."""
+    su, oracle = mods
+    dims = (L,) * 4
+    G = su.Lattice(Nc, dims, precision, kernel=kernel)
+    O = oracle.OracleLattice(Nc, dims, precision)
+    (G.init_hot if start == "hot" else G.init_cold)(seed)
+    (O.init_hot if start == "hot" else O.init_cold)(seed)
+    assert _maxdiff(G.export_links(), O.export_links()) <= (1e-12 if precision == "fp64" else 3e-7)
+    O.sweep(beta, 1, 1)
+    lo = O.export_links()
+    G.import_links(lo)
+    G.set_rng(seed, 1)
+    tol = 1e-11 if precision == "fp64" else 2e-5
+    flipped = updated = 0
+    for kind, parity, mu in [(0, 0, 1), (0, 1, 3), (1, 1, 0), (1, 0, 2)]:
+        ag = G.substep(beta, kind, 0, parity, mu, want_attempts=(kind == 0))
+        ao = O.substep(beta, kind, 0, parity, mu, want_attempts=(kind == 0))
+        lg, lo = G.export_links(), O.export_links()
+        sites = _sites_of_parity(dims, parity)
+        d = np.abs(lg.reshape(-1, 4, Nc * Nc)[sites, mu] - lo.reshape(-1, 4, Nc * Nc)[sites, mu]).max(axis=1)
+        mism = np.zeros(len(sites), dtype=bool)
+        if kind == 0:
+            mism = (ag != ao).any(axis=0)
+            assert ao.min() >= 1
+            if precision == "fp64":
+                assert not mism.any()
+        flipped += int(mism.sum())
+        updated += len(sites)
+        assert d[~mism].max() <= tol, (kind, parity, mu, float(d[~mism].max()))
+        assert _maxdiff(lg, lo) <= (tol if not mism.any() else 10.0)      # nothing else moved
+        G.import_links(lo)
+    assert flipped < 1e-5 * updated * Nc * (Nc - 1) / 2 + 1
+    assert G.counters()[1] == 0

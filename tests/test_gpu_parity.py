@@ -322,3 +322,122 @@ def test_error_codes(mods):
         assert e.value.status == su.SU_EINVAL
     G.sweep(6.0, 0, 0)                         # empty sweep is legal
     assert G.plaquette() == 1.0
+
+
+@pytest.mark.parametrize("v", [(2, "fp64", False, "auto"), (3, "fp64", False, "auto"), (3, "fp32", True, "auto"),
+                               (4, "fp64", False, "auto"), (6, "fp64", False, "auto")], ids=_ids)
+@pytest.mark.parametrize("zc", [1, 2, 4])
+def test_forced_z_chunk_traversal(mods, v, zc):
+    """The z-chunked traversal order (Zc < Lz; at the default 16 MB rule only the 48^4 lattice chunks) forced on
+    the small anisotropic lattice through su_set_option("z_chunk_planes"): a sweep, the reunitarisation and the
+    plaquette must be BITWISE what the unchunked traversal gives (the order only permutes independent threads),
+    and a lock-step heatbath + overrelaxation sub-step must match the oracle, attempt counts included."""
+    su, _ = mods
+    Nc, precision, recon12, kernel = v
+    A = su.Lattice(Nc, DIMS_ANISO, precision, recon12, kernel)
+    B = su.Lattice(Nc, DIMS_ANISO, precision, recon12, kernel)
+    assert A.get_option("z_chunk_planes") == DIMS_ANISO[2]
+    B.set_option("z_chunk_planes", zc)
+    assert B.get_option("z_chunk_planes") == zc
+    with pytest.raises(su.SuError):
+        B.set_option("z_chunk_planes", 3)                     # does not divide Lz = 8
+    with pytest.raises(su.SuError):
+        B.set_option("no_such_knob", 1)
+    A.init_hot(3)
+    B.init_hot(3)
+    for _ in range(2):
+        A.sweep(BETA[Nc], 1, 2)
+        B.sweep(BETA[Nc], 1, 2)
+        if Nc > 2:
+            A.reunitarize()
+            B.reunitarize()
+    assert np.array_equal(A.export_links(), B.export_links())
+    assert A.plaquette() == B.plaquette()                     # the plaquette kernel walks the same chunks
+    assert A.counters() == B.counters()
+    O = mods[1].OracleLattice(Nc, DIMS_ANISO, precision, recon12)
+    O.import_links(B.export_links())
+    O.set_rng(3, 2)
+    B.import_links(O.export_links())
+    for kind, parity, mu in [(0, 1, 2), (1, 0, 3), (0, 0, 1)]:
+        ag = B.substep(BETA[Nc], kind, 0, parity, mu, want_attempts=True)
+        ao = O.substep(BETA[Nc], kind, 0, parity, mu, want_attempts=True)
+        lg, lo = B.export_links(), O.export_links()
+        flips = (ag != ao).any(axis=0)
+        d = np.abs(lg - lo).reshape(-1, 4, Nc * Nc).max(axis=2)
+        bad = np.zeros(O.V, dtype=bool)
+        bad[_sites_of_parity(DIMS_ANISO, parity)[flips]] = True
+        assert d[~bad].max() <= TOL[precision]
+        assert bad.sum() <= (0 if precision == "fp64" else 1)
+        B.import_links(lo)
+
+
+@pytest.mark.parametrize("v", [(2, "fp64", False, "auto"), (3, "fp64", False, "auto"), (4, "fp32", False, "auto"),
+                               (5, "fp64", False, "auto")], ids=_ids)
+def test_heatbath_pass_number_enters_the_draws(mods, v):
+    """Several heatbath passes per sweep: the pass number is a field of the Philox counter (DESIGN.md "RNG
+    keying"); sub-steps with pass 1, 7 and 255 must draw what the oracle draws (attempt counts per link and
+    subgroup equal) and differ from pass 0."""
+    Nc, precision, recon12, kernel = v
+    G, O = _pair(mods, Nc, DIMS_ANISO, precision, recon12, kernel)
+    O.init_hot(21)
+    O.sweep(BETA[Nc], 1, 1)
+    start = O.export_links()
+    outs = {}
+    for pass_ in (0, 1, 7, 255):
+        G.import_links(start)
+        O.import_links(start)
+        G.set_rng(21, 5)
+        O.set_rng(21, 5)
+        ag = G.substep(BETA[Nc], 0, pass_, 1, 2, want_attempts=True)
+        ao = O.substep(BETA[Nc], 0, pass_, 1, 2, want_attempts=True)
+        lg, lo = G.export_links(), O.export_links()
+        flips = (ag != ao).any(axis=0)
+        assert flips.sum() <= (0 if precision == "fp64" else 1)
+        bad = np.zeros(O.V, dtype=bool)
+        bad[_sites_of_parity(DIMS_ANISO, 1)[flips]] = True
+        d = np.abs(lg - lo).reshape(-1, 4, Nc * Nc).max(axis=2)
+        assert d[~bad].max() <= TOL[precision]
+        outs[pass_] = lg
+    for p in (1, 7, 255):
+        assert np.abs(outs[p] - outs[0]).max() > 1e-3
+
+
+def test_sweep_with_two_heatbath_passes_matches_the_oracle(mods):
+    G, O = _pair(mods, 3, DIMS_ANISO, "fp64", False, "auto")
+    n = _thermalised_oracle(O, 3)
+    G.import_links(O.export_links())
+    G.set_rng(11, n)
+    G.sweep(6.0, 2, 1)
+    O.sweep(6.0, 2, 1)
+    assert np.abs(G.export_links() - O.export_links()).max() <= 1e-11
+
+
+def test_state_checks_of_timing_and_graph_mode(mods):
+    su, _ = mods
+    G = su.Lattice(3, DIMS_TINY)
+    G.init_cold(1)
+    G.set_timing(True)
+    with pytest.raises(su.SuError) as e:
+        G.set_graph_mode(True)
+    assert e.value.status == su.SU_EUNSUPPORTED
+    G.set_timing(False)
+    G.set_graph_mode(True)
+    with pytest.raises(su.SuError) as e:
+        G.set_timing(True)
+    assert e.value.status == su.SU_EUNSUPPORTED
+    G.sweep(6.0, 1, 1)
+
+
+def test_graph_mode_follows_a_new_seed(mods):
+    """The Philox key is baked into captured launches: su_init_* with another seed must drop the cached graphs
+    (ADVICE round 1), so graph replay stays bitwise equal to plain launches."""
+    su, _ = mods
+    outs = []
+    for graph in (False, True):
+        G = su.Lattice(3, DIMS_ANISO, "fp64", graph=graph)
+        G.init_hot(5)
+        G.sweep(6.0, 1, 1)
+        G.init_hot(6)
+        G.sweep(6.0, 1, 1)
+        outs.append(G.export_links())
+    assert np.array_equal(outs[0], outs[1])

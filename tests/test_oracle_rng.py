@@ -143,3 +143,106 @@ def test_kp_acceptance_rates():
 def test_kp_unusable_alpha_is_reported():
     v, att = oracle.kp_sample(0.0, seed=1, n=4)
     assert np.all(att == 0)
+
+
+# ---- placement of every field of the Philox counter ---------------------------
+# An independent statement of one heatbath link update, written from the documented keying
+#   c0 = lexicographic site, c1 = sweep counter, c2 = kind<<28 | pass<<20 | parity<<19 | mu<<17 | subgroup,
+#   c3 = attempt number (kind 0) / 0 (kind 1 = direction), key = (seed low, seed high)
+# with the big-integer Philox above (pinned by the KATs) and numpy fp64. From a COLD start every staple is
+# 6 * 1 and every link is 1, so the link a heatbath sub-step leaves at a site depends on nothing but the
+# random numbers of that (site, sweep, pass, parity, mu, subgroup, attempt): two fields sharing a bit, a field
+# left out of the counter, or a wrong shift changes them.
+def _np_uniform(w):
+    return (w + 1) / 4294967296.0
+
+
+def _np_kp(alpha, key, c0, c1, c2_low):
+    for n in range(1024):
+        w = _philox_bigint((c0, c1, c2_low | (0 << 28), n), key)
+        r1, r2, r3, r4 = (_np_uniform(x) for x in w)
+        c = np.cos(2 * np.pi * r2)
+        lam2 = -(np.log(r1) + c * c * np.log(r3)) / (2 * alpha)
+        if r4 * r4 <= 1 - lam2:
+            a0 = 1 - 2 * lam2
+            break
+    else:
+        raise AssertionError("no acceptance")
+    d = _philox_bigint((c0, c1, c2_low | (1 << 28), 0), key)
+    cos_t = 1 - 2 * _np_uniform(d[0])
+    sin_t = np.sqrt(max(0.0, 1 - cos_t * cos_t))
+    phi = 2 * np.pi * _np_uniform(d[1])
+    rho = np.sqrt(max(0.0, 1 - a0 * a0))
+    return np.array([a0, rho * sin_t * np.cos(phi), rho * sin_t * np.sin(phi), rho * cos_t]), n + 1
+
+
+def _np_heatbath_link_from_cold(Nc, beta, seed, site, sweep, pass_, parity, mu):
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    U = np.eye(Nc, dtype=complex)
+    W = 6.0 * np.eye(Nc, dtype=complex)                    # U S^dagger with S = 6 * 1
+    q = 0
+    attempts = []
+    for i in range(Nc - 1):
+        for j in range(i + 1, Nc):
+            r = 0.5 * np.array([(W[i, i] + W[j, j]).real, (W[i, j] + W[j, i]).imag,
+                                (W[i, j] - W[j, i]).real, (W[i, i] - W[j, j]).imag])      # eq 11
+            k = np.sqrt((r * r).sum())
+            ud = np.array([r[0], -r[1], -r[2], -r[3]]) / k
+            c2_low = (pass_ << 20) | (parity << 19) | (mu << 17) | q
+            v, used = _np_kp(2 * beta * k / Nc, key, site, sweep, c2_low)
+            attempts.append(used)
+            a = np.array([v[0] * ud[0] - v[1:] @ ud[1:],
+                          *(v[0] * ud[1:] + ud[0] * v[1:] - np.cross(v[1:], ud[1:]))])       # a = v u~^dagger (eq 14)
+            A = np.eye(Nc, dtype=complex)
+            A[i, i], A[i, j] = a[0] + 1j * a[3], a[2] + 1j * a[1]                          # eq 6
+            A[j, i], A[j, j] = -a[2] + 1j * a[1], a[0] - 1j * a[3]
+            U, W = A @ U, A @ W                                                            # eq 15
+            q += 1
+    return U, attempts
+
+
+@pytest.mark.parametrize("Nc,beta", [(2, 2.3), (3, 6.0), (4, 11.0)])
+def test_counter_field_placement_against_an_independent_statement(Nc, beta):
+    dims = (2, 2, 2, 4)
+    V = int(np.prod(dims))
+    cases = [(0x1_0000_0007, 0, 0, 0, 0), (7, 9, 0, 1, 3), (7, 0, 3, 0, 2), (7, 0, 255, 1, 1), (7, 0, 1, 1, 0),
+             (7, 1, 0, 0, 1)]
+    seen = {}
+    for seed, sweep, pass_, parity, mu in cases:
+        L = oracle.OracleLattice(Nc, dims)
+        L.init_cold(0)
+        L.set_rng(seed, sweep)
+        att = L.substep(beta, 0, pass_, parity, mu, want_attempts=True)
+        links = L.export_links().reshape(V, 4, Nc, Nc)
+        t, z, y, x = np.unravel_index(np.arange(V), dims[::-1])
+        sites = np.nonzero((x + y + z + t) % 2 == parity)[0]
+        for s in (sites[0], sites[3], sites[-1]):
+            U, used = _np_heatbath_link_from_cold(Nc, beta, seed, int(s), sweep, pass_, parity, mu)
+            assert np.abs(links[s, mu] - U).max() < 1e-12, (seed, sweep, pass_, parity, mu, s)
+            assert list(att[:, s // 2]) == used
+            seen[(seed, sweep, pass_, parity, mu, int(s))] = U
+        L.close()
+    # distinct key tuples give distinct links (no two of the cases above collide)
+    vals = list(seen.values())
+    for i in range(len(vals)):
+        for j in range(i + 1, len(vals)):
+            assert np.abs(vals[i] - vals[j]).max() > 1e-6
+
+
+def test_counter_word_c2_fields_do_not_overlap():
+    """The documented packing itself: 17 bits of subgroup, 2 of mu, 1 of parity, 8 of pass, 4 of kind are
+    disjoint, so distinct (kind, pass, parity, mu, subgroup) are distinct 32-bit words."""
+    words = set()
+    n = 0
+    for kind in (0, 1, 2):
+        for pass_ in (0, 1, 2, 128, 255):
+            for parity in (0, 1):
+                for mu in range(4):
+                    for sub in (0, 1, 2, 5, 14, 27, 119, 495, (1 << 17) - 1):
+                        words.add((kind << 28) | (pass_ << 20) | (parity << 19) | (mu << 17) | sub)
+                        n += 1
+    assert len(words) == n
+    base = oracle.philox4x32_10((3, 1, 0, 0), (5, 6))
+    for w in list(words)[:200]:
+        if w:
+            assert oracle.philox4x32_10((3, 1, w, 0), (5, 6)) != base
