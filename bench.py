@@ -152,8 +152,13 @@ def whole_job_rate(world, updates_per_rank_step, ms, steps):
     return world * updates_per_rank_step / (ms / steps * 1e-3)
 
 
+OPTIONS = {}          # --option name=value: su_set_option knobs applied to every lattice of the run
+
+
 def make_lattice(su, wl, precision, recon12, kernel, rank, device):
     lat = su.Lattice(wl["Nc"], (wl["L"],) * 4, precision, recon12=recon12, kernel=kernel, device=device)
+    for k, v in OPTIONS.items():
+        lat.set_option(k, v)
     if wl["start"] == "hot":
         lat.init_hot(rank_seed(wl, rank))
     else:
@@ -174,7 +179,21 @@ def time_resident(torch, dist, lat, wl, steps, warmup, sample_clocks, gpu_index)
     reunit = wl["Nc"] > 2
     for _ in range(warmup):
         one_step(lat, wl["beta"], reunit)
-    lat.set_timing(True)
+    # L2-resident lattices are launch-bound: the per-kind kernel times (roofline) come from a short pass of plain
+    # launches, the timed steps then replay each sweep as ONE CUDA graph (su_set_graph_mode; the two cannot be combined)
+    graph = lat.links_bytes < 96e6 and not lat.slab
+    tim = None
+    if graph:
+        lat.set_timing(True)
+        for _ in range(min(steps, 5)):
+            one_step(lat, wl["beta"], reunit)
+        tim = lat.timing()
+        lat.set_timing(False)
+        lat.set_graph_mode(True)
+        for _ in range(3):
+            one_step(lat, wl["beta"], reunit)
+    else:
+        lat.set_timing(True)
     n0 = lat.launch_count()
     if dist is not None:
         dist.barrier()
@@ -192,12 +211,13 @@ def time_resident(torch, dist, lat, wl, steps, warmup, sample_clocks, gpu_index)
         dist.barrier()
     ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop(t0, t1) if sampler else None
-    tim = lat.timing()
-    lat.set_timing(False)
+    if not graph:
+        tim = lat.timing()
+        lat.set_timing(False)
     launches = lat.launch_count() - n0
     att, exh = lat.counters()
     return dict(ms=ms, wall_ms=(t1 - t0) * 1e3, clocks=clocks, timing=tim, launches=launches, plaquette=plaq,
-                polyakov=[poly.real, poly.imag], kp_exhausted=exh)
+                polyakov=[poly.real, poly.imag], kp_exhausted=exh, graph=graph)
 
 
 def time_e2e(torch, dist, lat, wl, steps):
@@ -344,6 +364,119 @@ def run_nc_scan(args, torch, su, local):
     return 0
 
 
+CONFIG_RUNS = [   # BASELINE.json configs, as stated there: (tag, workload, sweeps, [(precision, recon12, kernel)], oracle sweeps)
+    ("C1", "su2_8", 20, [("fp64", False, "auto")], 20),
+    ("C2", "su3_16", 200, [("fp64", False, "auto"), ("fp64", True, "auto"), ("fp32", False, "auto"), ("fp32", True, "auto")], 200),
+    ("C3", "su3_48", 100, [("fp64", False, "auto"), ("fp64", True, "auto"), ("fp32", False, "auto"), ("fp32", True, "auto")], 2),
+    ("C4", "su4_24", 100, [("fp64", False, "auto"), ("fp64", False, "generic"), ("fp32", False, "auto"), ("fp32", False, "generic")], 5),
+    ("C5", "su6_16", 50, [("fp64", False, "auto")], 50),
+]
+
+
+def run_config_table(args, torch, su, local, peak):
+    """--config-table: every BASELINE.json config run as stated there (sweep counts, reunitarisation per sweep for
+    Nc >= 3, plaquette (and Polyakov loop) per sweep), GPU and oracle side by side. One JSON line per (config, variant)
+    and a markdown table at the end (committed under profiles/ and quoted in BASELINE.md section 3). The oracle runs the
+    whole chain where that takes seconds to a minute (C1, C2, C5: the plaquette histories are compared sweep by
+    sweep) and a bounded number of sweeps otherwise (C3: 2, C4: 5), always the first variant of the config."""
+    import numpy as np
+    import oracle
+    rows = []
+    for tag, wname, n_sweeps, variants, n_oracle in CONFIG_RUNS:
+        if args.workload != "su3_48" and args.workload != wname:
+            continue
+        wl = WORKLOADS[wname]
+        Nc, V = wl["Nc"], wl["L"] ** 4
+        reunit = Nc > 2
+        warm = 20 if tag == "C3" else 0
+        o_hist, o_rate, o_threads = None, None, None
+        for vi, (precision, r12, kernel) in enumerate(variants):
+            lat = su.Lattice(Nc, (wl["L"],) * 4, precision, recon12=r12, kernel=kernel, device=local)
+            for k, v in OPTIONS.items():
+                lat.set_option(k, v)
+            (lat.init_hot if wl["start"] == "hot" else lat.init_cold)(wl["seed"])
+            if lat.links_bytes < 96e6:
+                lat.set_graph_mode(True)
+            for _ in range(warm):
+                lat.sweep(wl["beta"], N_HB, N_OR)
+                if reunit:
+                    lat.reunitarize()
+            torch.cuda.synchronize()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            hist, poly = [], []
+            t_meas = 0.0
+            ev0.record(lat.stream)
+            for _ in range(n_sweeps):
+                lat.sweep(wl["beta"], N_HB, N_OR)
+                if reunit:
+                    lat.reunitarize()
+                hist.append(lat.plaquette())
+                if tag == "C5":
+                    poly.append(abs(lat.polyakov()))
+            ev1.record(lat.stream)
+            torch.cuda.synchronize()
+            ms = ev0.elapsed_time(ev1) / n_sweeps                     # per sweep, measurements included
+            # per-kind kernel times from a short pass of plain launches
+            lat.set_graph_mode(False)
+            lat.set_timing(True)
+            for _ in range(3):
+                lat.sweep(wl["beta"], N_HB, N_OR)
+            tim = lat.timing()
+            lat.set_timing(False)
+            or_ms, hb_ms = tim["or_ms"] / tim["or_launches"], tim["hb_ms"] / tim["hb_launches"]
+            bpu = algorithmic_bytes_per_update(Nc, precision, r12)
+            gbs = bpu * (V // 2) / (or_ms * 1e-3) / 1e9
+            tf = flops_per_update(Nc, "or", r12) * (V // 2) / (or_ms * 1e-3) / 1e12
+            flops_sweep = 4 * V * (N_HB * flops_per_update(Nc, "hb", r12) + N_OR * flops_per_update(Nc, "or", r12))
+            if vi == 0:                                              # the oracle beside it, same start
+                O = oracle.OracleLattice(Nc, (wl["L"],) * 4, precision, r12)
+                (O.init_hot if wl["start"] == "hot" else O.init_cold)(wl["seed"])
+                o_hist = []
+                t0 = time.perf_counter()
+                for i in range(n_oracle):
+                    O.sweep(wl["beta"], N_HB, N_OR)
+                    if reunit:
+                        O.reunitarize()
+                    o_hist.append(O.plaquette())
+                    if time.perf_counter() - t0 > 150.0:
+                        break
+                o_rate = len(o_hist) * (N_HB + N_OR) * 4 * V / (time.perf_counter() - t0)
+                o_threads = oracle.num_threads()
+                O.close()
+            n_cmp = min(len(o_hist), len(hist)) if vi == 0 and warm == 0 else 0
+            row = {"config": tag, "workload": wname, "Nc": Nc, "lattice": f"{wl['L']}^4", "precision": precision,
+                   "storage": "12-real" if r12 else ("4-real" if Nc == 2 else f"{2 * Nc * Nc}-real"), "kernel": kernel,
+                   "beta": wl["beta"], "start": f"{wl['start']} seed {wl['seed']}", "sweeps": n_sweeps, "warmup_sweeps": warm,
+                   "ms_per_sweep": ms, "link_updates_per_s": (N_HB + N_OR) * 4 * V / (ms * 1e-3),
+                   "gflops": flops_sweep / (ms * 1e-3) / 1e9, "or_substep_ms": or_ms, "hb_substep_ms": hb_ms,
+                   "or_hbm_frac_measured_peak": gbs / peak[0], "or_hbm_frac_8TBs": gbs / 8000.0,
+                   "or_alu_frac": tf / FMA_PEAKS[precision], "plaquette_last": hist[-1],
+                   "plaquette_mean_last_half": float(np.mean(hist[len(hist) // 2:])),
+                   "polyakov_abs_last": poly[-1] if poly else None,
+                   "oracle_link_updates_per_s": o_rate if vi == 0 else None, "oracle_threads": o_threads if vi == 0 else None,
+                   "oracle_sweeps": len(o_hist) if vi == 0 else None,
+                   "max_abs_dP_first_3_sweeps": float(np.abs(np.array(hist[:3]) - np.array(o_hist[:3])).max()) if n_cmp >= 3 else None,
+                   "oracle_plaquette_mean_last_half": float(np.mean(o_hist[len(o_hist) // 2:])) if vi == 0 and n_cmp == len(hist) else None,
+                   "graph_replay": lat.links_bytes < 96e6}
+            rows.append(row)
+            print(json.dumps(row), flush=True)
+            lat.close()
+    print("\n| config | group, lattice | precision, storage, kernel | ms / sweep | G link updates/s | TFLOP/s | OR sub-step ms | HB sub-step ms | "
+          "OR frac of HBM (measured / 8 TB/s) | OR frac of FMA peak | oracle M updates/s (threads) | plaquette (GPU; oracle) |")
+    print("|---|---|---|---:|---:|---:|---:|---:|---:|---:|---:|---|")
+    for r in rows:
+        orc = f"{r['oracle_link_updates_per_s'] / 1e6:.2f} ({r['oracle_threads']}; {r['oracle_sweeps']} sweeps)" if r["oracle_link_updates_per_s"] else ""
+        pl = f"{r['plaquette_mean_last_half']:.5f}"
+        if r["oracle_plaquette_mean_last_half"] is not None:
+            pl += f"; {r['oracle_plaquette_mean_last_half']:.5f}"
+        if r["max_abs_dP_first_3_sweeps"] is not None:
+            pl += f" (first 3 sweeps agree to {r['max_abs_dP_first_3_sweeps']:.1e})"
+        print(f"| {r['config']} | SU({r['Nc']}) {r['lattice']} | {r['precision']}, {r['storage']}, {r['kernel']} | {r['ms_per_sweep']:.3f} | "
+              f"{r['link_updates_per_s'] / 1e9:.3f} | {r['gflops'] / 1e3:.2f} | {r['or_substep_ms']:.4f} | {r['hb_substep_ms']:.4f} | "
+              f"{r['or_hbm_frac_measured_peak']:.2f} / {r['or_hbm_frac_8TBs']:.2f} | {r['or_alu_frac']:.2f} | {orc} | {pl} |")
+    return 0
+
+
 def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
     """--parallel slabs: ONE lattice, rank r owns the time slices [r Lt/N, (r+1) Lt/N). Step =
     40 sub-steps (each followed by the stream-ordered rank ordering) + reunitarise + plaquette (all-reduce). The
@@ -399,8 +532,15 @@ def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
     return 0
 
 
+FMA_PEAKS = {}        # precision -> measured TFLOP/s of the FMA pipe (su_measure_fma_peak), filled once per run
+
+
 def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
-    """Turn one timed run into the metric, GFLOPS and the roofline object of its dominant (OR) kernel."""
+    """Turn one timed run into the metric, GFLOPS and the roofline object of its dominant (OR) kernel.
+    Two roofs are evaluated for the overrelaxation sub-step: HBM (9 R s bytes per update, against the
+    measured copy bandwidth) and ALU (the stated flop count per update against the FMA rate measured in this run by
+    su_measure_fma_peak: 64 FP64 / 128 FP32 FMAs per clock and SM at the clock of a short burst); `bound` names the
+    roof the kernel sits closer to (the larger fraction), both fractions are reported."""
     Nc, V = wl["Nc"], wl["L"] ** 4
     updates_step = (N_HB + N_OR) * 4 * V
     t_step = res["ms"] / steps * 1e-3
@@ -413,13 +553,26 @@ def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
         or_ms = tim["or_ms"] / tim["or_launches"]
         hb_ms = tim["hb_ms"] / tim["hb_launches"] if tim["hb_launches"] else None
         ach = bpu * (V // 2) / (or_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k_update (overrelaxation sub-step; 32 of the 40 update launches per sweep)",
-                "achieved": ach, "peak": peak[0], "unit": "GB/s", "frac": ach / peak[0], "peak_source": peak[1],
+        f_or = flops_per_update(Nc, "or", recon12)
+        tf = f_or * (V // 2) / (or_ms * 1e-3) / 1e12
+        alu_peak = FMA_PEAKS.get(precision)
+        frac_hbm, frac_alu = ach / peak[0], (tf / alu_peak if alu_peak else None)
+        alu_bound = frac_alu is not None and frac_alu > frac_hbm
+        roof = {"bound": "alu" if alu_bound else "hbm",
+                "kernel": "staple + overrelaxation update, one (parity, mu) sub-step (32 of the 40 update sub-steps per sweep)",
+                "achieved": tf if alu_bound else ach, "peak": alu_peak if alu_bound else peak[0],
+                "unit": "TFLOP/s" if alu_bound else "GB/s", "frac": frac_alu if alu_bound else frac_hbm,
+                "peak_source": "measured in this run (su_measure_fma_peak, burst clock)" if alu_bound else peak[1],
+                "hbm": {"achieved_gbs": ach, "peak_gbs": peak[0], "frac": frac_hbm, "frac_of_8TBs": ach / 8000.0,
+                        "bytes_per_link_update": bpu, "algorithmic_bytes_per_launch": bpu * (V // 2)},
+                "alu": {"achieved_tflops": tf, "peak_tflops": alu_peak, "frac": frac_alu, "flops_per_link_update": f_or},
                 "frac_of_8TBs": ach / 8000.0, "algorithmic_bytes_per_launch": bpu * (V // 2),
                 "bytes_per_link_update": bpu, "avg_launch_ms": or_ms, "hb_avg_launch_ms": hb_ms,
                 "hb_achieved": (bpu * (V // 2) / (hb_ms * 1e-3) / 1e9) if hb_ms else None,
-                "update_kernels_share_of_step": (tim["or_ms"] + tim["hb_ms"]) / res["ms"],
-                "traffic": ncu_traffic(f"su{Nc}_{precision}_{'recon12' if recon12 else 'full'}_or")}
+                "hb_alu_frac": (flops_per_update(Nc, "hb", recon12) * (V // 2) / (hb_ms * 1e-3) / 1e12 / alu_peak) if hb_ms and alu_peak else None,
+                "update_kernels_share_of_step": ((or_ms * N_OR * 8 + (hb_ms or 0.0) * N_HB * 8) / (res["ms"] / steps)),
+                "traffic": ncu_traffic(f"su{Nc}_{precision}_{'recon12' if recon12 else 'full'}_or"),
+                "traffic_source": "profiles/traffic.csv (ncu --set full of this kernel, committed; not re-measured in this run)"}
     return {"value": value, "ms_per_step": res["ms"] / steps, "gflops": n_ranks * flops_step / t_step / 1e9,
             "effective_gbs": n_ranks * bpu * updates_step / t_step / 1e9, "roofline": roof}
 
@@ -434,18 +587,26 @@ def main():
     ap.add_argument("--storage", default="full", choices=["full", "recon12"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "specialised", "generic"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
-                    help="N > 1: independent replicas (default; weak scaling) or ONE lattice cut into N t-slabs with "
-                         "halo pushes over peer memory (strong scaling; DESIGN.md 9)")
+    ap.add_argument("--parallel", default="auto", choices=["auto", "replicas", "slabs"],
+                    help="N > 1: ONE lattice cut into N t-slabs with halo pushes over peer memory (the default when N > 1: "
+                         "the path that shards, strong scaling; DESIGN.md 9) or independent replicas (weak scaling, on request)")
     ap.add_argument("--nc-scan", action="store_true",
                     help="the paper's Nc-scaling study (PAPER.md:295-303, Figs 11-12): time per iteration (1 heatbath + 1 "
                          "overrelaxation + reunitarise + plaquette) vs Nc at 8^4 and 16^4, beta 6.2, generic and specialised")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
+                    help="su_set_option knob for every lattice of the run (e.g. fuse=2); recorded in config.options")
+    ap.add_argument("--config-table", action="store_true",
+                    help="run the five BASELINE.json configs as stated there (sweep counts, histories), GPU and oracle side by "
+                         "side; JSON lines plus a markdown table (BASELINE.md section 3). --workload X restricts it to one config")
     ap.add_argument("--no-variants", action="store_true", help="skip the extra fp32 / 12-real runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
     wl = WORKLOADS[args.workload]
+    for kv in args.option:
+        k, v = kv.split("=", 1)
+        OPTIONS[k] = int(v)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -466,6 +627,12 @@ def main():
     recon12 = args.storage == "recon12"
     if args.nc_scan:
         return run_nc_scan(args, torch, su, local)
+    if args.parallel == "auto":
+        args.parallel = "slabs" if world > 1 else "replicas"
+    for prec in {args.precision, "fp32", "fp64"}:
+        FMA_PEAKS[prec] = su.measure_fma_peak(prec, local)[0]
+    if args.config_table:
+        return run_config_table(args, torch, su, local, peak)
     if args.parallel == "slabs":
         if dist is None:                          # a single rank still goes through the slab path (one slab, self-peered)
             import torch.distributed as dist
@@ -521,13 +688,15 @@ def main():
                            "start": f"{wl['start']} (Philox seed {wl['seed']} + rank)", "sweep": "1 heatbath + 4 overrelaxation",
                            "step": "su_sweep(1,4) + su_reunitarize + su_plaquette + su_polyakov" if wl["Nc"] > 2
                                    else "su_sweep(1,4) + su_plaquette + su_polyakov",
-                           "storage": args.storage, "kernel": args.kernel,
+                           "storage": args.storage, "kernel": args.kernel, "options": dict(OPTIONS), "library": su.LIB_PATH,
+                           "graph_replay": bool(res.get("graph")),
                            "lattice_bytes": su.lattice_bytes(wl["Nc"], (wl["L"],) * 4, args.precision, recon12),
                            "l2": "inputs larger than L2 (no flush)" if su.lattice_bytes(wl["Nc"], (wl["L"],) * 4, args.precision, recon12) > 3 * 126e6
                                  else "lattice fits in L2: L2-resident by design, HBM fraction not meaningful",
                            "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)"},
                 "gflops": main_num["gflops"], "effective_hbm_gbs": main_num["effective_gbs"],
                 "flop_formula": "13*mm+10Nc^2 + n_sub*(23+56Nc) [OR] / n_sub*(57+13*1.05+56Nc) [HB], mm=8Nc^3-2Nc^2 (DESIGN.md)",
+                "fma_peaks_tflops": dict(FMA_PEAKS),
                 "roofline": main_num["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": res["launches"],
                 "clocks": res["clocks"], "plaquette": res["plaquette"], "polyakov": res["polyakov"],
                 "kp_exhausted": res["kp_exhausted"], "variants": variants}

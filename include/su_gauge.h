@@ -51,7 +51,7 @@ typedef enum {
     SU_KERNEL_GENERIC = 2      /* the generic SU(Nc) kernel at any supported Nc */
 } su_kernel;
 
-#define SU_MAX_NC 8
+#define SU_MAX_NC 32 /* Nc <= 8: kernels compiled per Nc; 9..32: the runtime-Nc warp-per-link kernels */
 
 typedef struct {
     su_storage storage;
@@ -83,7 +83,7 @@ su_status su_init_hot(su_lattice*, uint64_t seed);
  * (eqs 9-16) followed by n_overrelax overrelaxation passes (eq 17); each pass updates every link
  * once, as 8 sub-steps: parity 0,1 (outer) x mu 0..3 (inner). Wilson coupling beta = 2Nc/g^2
  * (eq 3). Asynchronous on the stream. Uses, then increments, the handle's sweep counter.
- * Never reunitarises. 0 <= n_heatbath <= 255, n_overrelax >= 0, beta finite and >= 0. */
+ * Never reunitarises (unless su_set_option "reunit_on_store" asks for it). 0 <= n_heatbath <= 255, n_overrelax >= 0, beta finite and >= 0. */
 su_status su_sweep(su_lattice*, double beta, int n_heatbath, int n_overrelax);
 
 /* Mean plaquette <ReTr P>/Nc over the 6V plaquettes (eq 4); fp64 accumulation.
@@ -100,6 +100,15 @@ su_status su_reunitarize(su_lattice*);
  * the third row. Synchronise. su_import_links marks the lattice initialised. */
 su_status su_export_links(su_lattice*, double* host_dst, size_t n_doubles);
 su_status su_import_links(su_lattice*, const double* host_src, size_t n_doubles);
+
+/* Configuration files ("file storing ... configurations"): a 64-byte header ("SUGCONF1", Nc, extents,
+ * precision, storage, RNG seed and sweep counter, plaquette), the links as canonical doubles (the su_export_links
+ * layout), and a 64-bit FNV-1a checksum of both. su_load_config needs a handle of the same Nc and extents (any
+ * precision / storage), verifies the checksum and that the plaquette it measures after the import matches the
+ * header, and restores the RNG seed and sweep counter: load + su_sweep continues the writer's chain exactly when
+ * precision and storage agree. Host-side I/O; both synchronise. Not available on slab handles. */
+su_status su_save_config(su_lattice*, const char* path);
+su_status su_load_config(su_lattice*, const char* path);
 
 /* ---- test / resume hooks ---- */
 /* Set the RNG seed and sweep counter: export + su_set_rng + import is an exact resume. */
@@ -121,7 +130,7 @@ su_status su_set_graph_mode(su_lattice*, int enabled);
 /* Per-kind device timing of su_sweep (for the benchmark's roofline): when enabled (and graph mode
  * is off) su_sweep records CUDA events on the handle's stream before the heatbath passes, between
  * the heatbath and overrelaxation passes, and after; su_get_timing synchronises and returns the
- * accumulated milliseconds and update-kernel launches per kind since su_set_timing.
+ * accumulated milliseconds and update SUB-STEPS per kind (8 per pass, however many launches ran them) since su_set_timing.
  * SU_EUNSUPPORTED in graph mode (events cannot be read back from a replayed graph). */
 su_status su_set_timing(su_lattice*, int enabled);
 su_status su_get_timing(su_lattice*, double* hb_ms, uint64_t* hb_launches, double* or_ms, uint64_t* or_launches);
@@ -166,9 +175,34 @@ su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* o
 /* ---- tuning knobs (none changes a result bit; DESIGN.md names the measured defaults) ----
  *   "z_chunk_planes"  z-planes per chunk of the update / plaquette kernels' traversal order (a divisor of Lz;
  *                     0 = the default rule: the largest chunk under 16 MB per time slice). Synchronises.
+ *   "fuse"            sub-steps of a pass that su_sweep runs in ONE launch: 1 (default here: one launch per
+ *                     (parity, mu), "eight steps"), 2, 4 or 8. Consecutive sub-steps read the same 4V
+ *                     links; run together while those are in L2 they move 8/g + 1 instead of 9 links per update.
+ *                     Blocks wait on per-(sub-step, cell) completion counters, so every update sees exactly the links
+ *                     it sees in the one-launch-per-sub-step sweep: the results are bitwise identical (tested).
+ *                     Ignored (plain launches) in slab mode and for kernels without a fused form; su_get_option
+ *                     "fuse_effective" tells what su_sweep will do.
+ *   "fuse_chunk_planes", "fuse_margin", "fuse_cell_planes"   shape of the fused schedule (csrc/fused_schedule.cu).
+ *   "reunit_on_store" 1: su_sweep leaves reunitarised links. Every link is updated exactly once in the last pass of
+ *                     a sweep; there the register kernels of Nc <= 4 project the link they have just updated back to
+ *                     SU(Nc) before they store it (PAPER.md:143 arithmetic, saving the separate read-modify-write of
+ *                     su_reunitarize); the other kernels run the reunitarisation kernel at the end of the sweep. This
+ *                     one DOES change results at rounding level against su_sweep + su_reunitarize (later sub-steps of
+ *                     the last pass already see projected neighbours); su_sweep without it never reunitarises. 0: off.
  * Unknown names: SU_EINVAL. */
 su_status su_set_option(su_lattice*, const char* name, long long value);
 su_status su_get_option(su_lattice*, const char* name, long long* value);
+
+/* Host-only views of the fused schedule, for the CPU test that proves it (tests/test_fused_schedule.py): the
+ * ticket table work[n_tickets][n_fused] (tile id = cell * nT + tile, 0xffffffff = none; cell = t * nzu + z-unit)
+ * with geom = {planes per cell, cells per time slice, tiles per cell, sites per cell, sites per plane}, and the
+ * k-th dependency (completion-counter index stage * cells + cell, or -1) of a work item, exactly as the kernel
+ * enumerates it. No device is touched. planes_per_cell / chunk_planes 0 = default. */
+su_status su_fused_schedule_debug(int Lx, int Ly, int Lz, int Lt, int sites_per_block, int n_fused, int first_substep,
+                                  int planes_per_cell, int chunk_planes, int margin, uint32_t* work, size_t work_capacity,
+                                  int* n_tickets, int* geom);
+int su_fused_dep_debug(int Lx, int Ly, int Lz, int Lt, int sites_per_block, int n_fused, int first_substep,
+                       int planes_per_cell, int stage, int cell, int tile, int k);
 
 /* Measured FMA rate of the device's FP32 / FP64 pipes in TFLOP/s (FMA = 2 flops): a short register-only
  * micro-benchmark (16 independent chains per thread, 8 blocks of 256 threads per SM, best of 5 launches of a few

@@ -22,7 +22,7 @@ _STATUS = {0: "SU_OK", 1: "SU_EINVAL", 2: "SU_EUNSUPPORTED", 3: "SU_ENOMEM", 4: 
 SU_FP32, SU_FP64 = 0, 1
 SU_STORE_FULL, SU_STORE_RECON12 = 0, 1
 SU_KERNEL_AUTO, SU_KERNEL_SPECIALISED, SU_KERNEL_GENERIC = 0, 1, 2
-SU_MAX_NC = 8
+SU_MAX_NC = 32
 
 # every entry point include/su_gauge.h declares (tests check the library exports exactly these)
 ABI_SYMBOLS = (
@@ -32,7 +32,7 @@ ABI_SYMBOLS = (
     "su_synchronize", "su_set_graph_mode", "su_set_timing", "su_get_timing", "su_get_launch_count", "su_last_error",
     "su_lattice_create_slab", "su_slab_bytes", "su_slab_links", "su_slab_set_peers", "su_slab_halo_push",
     "su_ipc_export", "su_ipc_open", "su_ipc_close", "su_slab_plaquette_sum", "su_set_option", "su_get_option",
-    "su_measure_fma_peak",
+    "su_measure_fma_peak", "su_save_config", "su_load_config", "su_fused_schedule_debug", "su_fused_dep_debug",
 )
 
 
@@ -93,6 +93,10 @@ def lib():
     L.su_ipc_open.argtypes = [P, C.c_char_p, C.POINTER(P)]
     L.su_ipc_close.argtypes = [P, P]
     L.su_slab_plaquette_sum.argtypes = [C.POINTER(P), I, C.POINTER(D)]
+    L.su_fused_schedule_debug.argtypes = [I] * 10 + [C.c_void_p, C.c_size_t, C.POINTER(I), C.POINTER(I)]
+    L.su_fused_dep_debug.argtypes = [I] * 12
+    L.su_save_config.argtypes = [P, C.c_char_p]
+    L.su_load_config.argtypes = [P, C.c_char_p]
     L.su_measure_fma_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D)]
     L.su_set_option.argtypes = [P, C.c_char_p, C.c_longlong]
     L.su_get_option.argtypes = [P, C.c_char_p, C.POINTER(C.c_longlong)]
@@ -158,6 +162,7 @@ class Lattice:
             nbytes = L.su_slab_bytes(self.Nc, *self.dims[:3], self.slab[1], _prec(precision), storage)
         if nbytes == 0:
             raise SuError(SU_EINVAL, "su_lattice_bytes", "invalid Nc / extents / storage")
+        self.links_bytes = int(nbytes)
         with torch.cuda.device(self.device):
             self.buffer = None if library_buffer else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = torch.cuda.current_stream(self.device)
@@ -242,6 +247,12 @@ class Lattice:
     def import_links(self, links):
         a = np.ascontiguousarray(links, dtype=np.complex128)
         self._ck(lib().su_import_links(self._h, a.ctypes.data, a.size * 2), "su_import_links")
+
+    def save_config(self, path):
+        self._ck(lib().su_save_config(self._h, str(path).encode()), "su_save_config")
+
+    def load_config(self, path):
+        self._ck(lib().su_load_config(self._h, str(path).encode()), "su_load_config")
 
     def counters(self):
         a, e = C.c_uint64(), C.c_uint64()

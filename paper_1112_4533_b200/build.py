@@ -22,11 +22,11 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
 ]
-HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", "update_rows_kernel.cuh", os.path.join("..", "..", "include", "su_gauge.h")]
+HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", "update_rows_kernel.cuh", "fused_schedule.h", os.path.join("..", "..", "include", "su_gauge.h")]
 
 
 def _units():
-    units = [("su_api.cu", None)]
+    units = [("su_api.cu", None), ("fused_schedule.cu", None), ("big_kernels.cu", None)]
     for nc in NCS:
         units.append(("update_kernels.cu", nc))
         units.append(("aux_kernels.cu", nc))

@@ -236,42 +236,6 @@ static __global__ void __launch_bounds__(REDUCE_BLOCK) k_reduce_final(const doub
     }
 }
 
-// ------------------------------------------------------------------------------------------
-// Gram-Schmidt / determinant on a local matrix (rolled loops), used by reunitarise (Nc >= 4)
-// and by the hot start (always double, reading R20).
-// ------------------------------------------------------------------------------------------
-template <int NC, class R, bool UNR = false>
-__device__ __forceinline__ void gram_schmidt_rows(cx<R>* U, int nrows) {
-#pragma unroll(UNR ? NC : 1)
-    for (int r = 0; r < (UNR ? NC : nrows); ++r) {
-#pragma unroll(UNR ? NC : 1)
-        for (int p = 0; p < r; ++p) {
-            cx<R> dot = mk<R>(0, 0);
-#pragma unroll(UNR ? NC : 1)
-            for (int k = 0; k < NC; ++k) mad_ca(dot, U[p * NC + k], U[r * NC + k]);
-#pragma unroll(UNR ? NC : 1)
-            for (int k = 0; k < NC; ++k) U[r * NC + k] = U[r * NC + k] - dot * U[p * NC + k];
-        }
-        R n2 = 0;
-#pragma unroll(UNR ? NC : 1)
-        for (int k = 0; k < NC; ++k) n2 += U[r * NC + k].re * U[r * NC + k].re + U[r * NC + k].im * U[r * NC + k].im;
-        R inv = (R)1 / Fn<R>::sqrt(n2);
-#pragma unroll(UNR ? NC : 1)
-        for (int k = 0; k < NC; ++k) U[r * NC + k] = inv * U[r * NC + k];
-    }
-}
-
-// det of a 4x4 complex matrix by the 2x2-minor (Laplace) expansion over rows {0,1} x {2,3}: no pivoting,
-// no dynamic indexing, so it stays in registers (used for the phase conj(det)/|det| only).
-template <class R>
-__device__ __forceinline__ cx<R> determinant4(const cx<R>* A) {
-    const cx<R> s0 = A[0] * A[5] - A[1] * A[4], s1 = A[0] * A[6] - A[2] * A[4], s2 = A[0] * A[7] - A[3] * A[4];
-    const cx<R> s3 = A[1] * A[6] - A[2] * A[5], s4 = A[1] * A[7] - A[3] * A[5], s5 = A[2] * A[7] - A[3] * A[6];
-    const cx<R> c5 = A[10] * A[15] - A[11] * A[14], c4 = A[9] * A[15] - A[11] * A[13], c3 = A[9] * A[14] - A[10] * A[13];
-    const cx<R> c2 = A[8] * A[15] - A[11] * A[12], c1 = A[8] * A[14] - A[10] * A[12], c0 = A[8] * A[13] - A[9] * A[12];
-    return (s0 * c5 - s1 * c4) + (s2 * c3 + s3 * c2) + (s5 * c0 - s4 * c1);
-}
-
 template <int NC, class R>
 __device__ cx<R> determinant(const cx<R>* A) {
     cx<R> Mx[NC * NC];
@@ -407,28 +371,6 @@ __global__ void __launch_bounds__(128) k_reunit_rows(const AuxArgs a) {
     }
 }
 
-// SU(3) rows 0,1 by modified Gram-Schmidt in registers (same operation order as gram_schmidt_rows)
-template <class T>
-__device__ __forceinline__ void gram_schmidt_su3_two_rows(cx<T>* U) {
-    T n2 = 0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) n2 += U[k].re * U[k].re + U[k].im * U[k].im;
-    T inv = (T)1 / Fn<T>::sqrt(n2);
-#pragma unroll
-    for (int k = 0; k < 3; ++k) U[k] = inv * U[k];
-    cx<T> dot = mk<T>(0, 0);
-#pragma unroll
-    for (int k = 0; k < 3; ++k) mad_ca(dot, U[k], U[3 + k]);
-#pragma unroll
-    for (int k = 0; k < 3; ++k) U[3 + k] = U[3 + k] - dot * U[k];
-    n2 = 0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) n2 += U[3 + k].re * U[3 + k].re + U[3 + k].im * U[3 + k].im;
-    inv = (T)1 / Fn<T>::sqrt(n2);
-#pragma unroll
-    for (int k = 0; k < 3; ++k) U[3 + k] = inv * U[3 + k];
-}
-
 // Reunitarisation (reading R10), arithmetic in T. Nc <= 4 runs in registers.
 template <int NC, class T, int STORE, bool UNR>
 __global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
@@ -438,20 +380,8 @@ __global__ void __launch_bounds__(128) k_reunit(const AuxArgs a) {
     typename IO::T2* pl = IO::plane(a.links, a.g, mu, p);
     cx<T> U[NC * NC];
     IO::template load<LD_STREAM>(pl, cb, U);
-    if (NC == 2) {
-        T n = Fn<T>::sqrt((U[0].re * U[0].re + U[0].im * U[0].im) + (U[1].re * U[1].re + U[1].im * U[1].im));
-        U[0] = mk<T>(U[0].re / n, U[0].im / n);
-        U[1] = mk<T>(U[1].re / n, U[1].im / n);
-    } else if (NC == 3) {
-        gram_schmidt_su3_two_rows<T>(U);
-        su3_third_row(U);
-    } else if (NC == 4) {
-        gram_schmidt_rows<NC, T, true>(U, NC);
-        const cx<T> d = determinant4<T>(U);
-        const T inv = (T)1 / Fn<T>::sqrt(d.re * d.re + d.im * d.im);
-        const cx<T> ph = mk<T>(d.re * inv, -d.im * inv);
-#pragma unroll
-        for (int k = 0; k < NC; ++k) U[(NC - 1) * NC + k] = U[(NC - 1) * NC + k] * ph;
+    if (NC <= 4) {
+        reunitarize_small<(NC <= 4 ? NC : 2), T>(U);        // (the conditional only keeps the dead branch of Nc > 4 compilable)
     } else {
         gram_schmidt_rows<NC, T>(U, NC);
         fix_determinant_phase<NC, T>(U);

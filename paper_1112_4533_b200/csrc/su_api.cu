@@ -1,6 +1,7 @@
 // su_api.cu — the C ABI of libsugauge (include/su_gauge.h): handle, validation, sweep schedule,
 // reductions' host side, import/export staging. All arithmetic of the method runs in the kernels
 // of update_kernels.cu / aux_kernels.cu; nothing here falls back to the CPU.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -37,12 +38,21 @@ struct su_lattice {
     size_t staging_bytes = 0;
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_filled[2] = {nullptr, nullptr}, ev_drained[2] = {nullptr, nullptr};
-    bool halos_valid = true;                     // slab mode: false between su_import_links and su_slab_halo_push
+    bool halos_valid = true;
+    // fused launches of g consecutive sub-steps (fused_schedule.h): tables per (g, stage pattern, tile size)
+    struct FusedTable { FusedGeom fg; unsigned n_tickets; uint32_t* d_work; unsigned* d_done; FusedCtrl* d_ctrl; };
+    std::map<std::tuple<int, int, int>, FusedTable> fused;
+    int fuse_g = 1;                  // sub-steps per launch: 1 (plain), 2, 4 or 8
+    int fuse_chunk_planes = 0;       // z-planes per chunk of the fused traversal (0: the plain kernel's Zc)
+    int fuse_margin = 8;             // tickets between a cell's last tile and the first tile that depends on it
+    int fuse_cell_planes = 0;        // z-planes per cell (0: chosen by fused_make_geom)
+    bool reunit_on_store = false;    // su_sweep leaves reunitarised links (in its last pass; see su_set_option)                     // slab mode: false between su_import_links and su_slab_halo_push
     uint64_t seed = 0;
     uint32_t sweep = 0;
     bool ready = false;
     bool graph_mode = false;
     std::map<std::tuple<double, int, int>, cudaGraphExec_t> graphs;
+    std::map<std::tuple<double, int, int>, uint64_t> graph_launches;    // kernels per replay of each graph
     uint64_t n_launch = 0;
     // per-kind device timing of su_sweep (su_set_timing): events before / between / after the pass groups
     bool timing = false;
@@ -126,7 +136,7 @@ int traversal_z_chunk(const Geom& g, size_t link_bytes) {
             case 6: return FN##6(__VA_ARGS__);                                 \
             case 7: return FN##7(__VA_ARGS__);                                 \
             case 8: return FN##8(__VA_ARGS__);                                 \
-            default: return cudaErrorInvalidValue;                             \
+            default: return FN##_big(__VA_ARGS__);        /* 9 .. SU_MAX_NC */ \
         }                                                                      \
     })()
 
@@ -161,13 +171,98 @@ __global__ void __launch_bounds__(256) k_fma_peak(T* out, const T* in, int iters
     if (s == (T)123456789) out[blockIdx.x * blockDim.x + threadIdx.x] = s;     // never true: keeps the chains alive
 }
 
+void free_fused(su_lattice* h) {
+    for (auto& kv : h->fused) {
+        cudaFree(kv.second.d_work); cudaFree(kv.second.d_done); cudaFree(kv.second.d_ctrl);
+    }
+    h->fused.clear();
+}
+
+int update_spb(su_lattice* h, int kind) {
+    switch (h->Nc) {
+        case 2: return update_spb_nc2(h->var, kind);
+        case 3: return update_spb_nc3(h->var, kind);
+        case 4: return update_spb_nc4(h->var, kind);
+        case 5: return update_spb_nc5(h->var, kind);
+        case 6: return update_spb_nc6(h->var, kind);
+        case 7: return update_spb_nc7(h->var, kind);
+        case 8: return update_spb_nc8(h->var, kind);
+        default: return 0;
+    }
+}
+
+// fused launches need the whole lattice in one buffer with periodic t (no slab halos) and a kernel that has the fused form
+int effective_fuse(su_lattice* h, int kind) {
+    if (h->fuse_g <= 1 || h->g.t_halo || update_spb(h, kind) <= 0) return 1;
+    return h->fuse_g;
+}
+
+// the table of the group of g sub-steps that starts at sub-step sub0 (built and uploaded on first use)
+su_status fused_table(su_lattice* h, int kind, int sub0, su_lattice::FusedTable** out) {
+    const int g = h->fuse_g, spb = update_spb(h, kind);
+    const auto key = std::make_tuple(g, sub0 % 4, spb);
+    auto it = h->fused.find(key);
+    if (it == h->fused.end()) {
+        su_lattice::FusedTable t{};
+        t.fg = fused_make_geom(h->g.L[0], h->g.L[1], h->g.L[2], h->g.L[3], spb, g, sub0 % 4, h->fuse_cell_planes);
+        const int chunk_planes = h->fuse_chunk_planes > 0 ? h->fuse_chunk_planes : h->g.Zc;
+        std::vector<uint32_t> work;
+        int nt = 0;
+        if (!fused_build_schedule(t.fg, chunk_planes / t.fg.U > 0 ? chunk_planes / t.fg.U : 1, h->fuse_margin, work, nt))
+            return fail(h, SU_ESTATE, "fused schedule construction failed");
+        t.n_tickets = (unsigned)nt;
+        const size_t ncnt = (size_t)g * t.fg.Lt * t.fg.nzu;
+        cudaError_t e = cudaMalloc(&t.d_work, work.size() * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMalloc(&t.d_done, ncnt * sizeof(unsigned));
+        if (e == cudaSuccess) e = cudaMalloc(&t.d_ctrl, sizeof(FusedCtrl));
+        if (e == cudaSuccess) e = cudaMemcpy(t.d_work, work.data(), work.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemset(t.d_done, 0, ncnt * sizeof(unsigned));
+        if (e == cudaSuccess) e = cudaMemset(t.d_ctrl, 0, sizeof(FusedCtrl));
+        if (e != cudaSuccess) {
+            cudaFree(t.d_work); cudaFree(t.d_done); cudaFree(t.d_ctrl); cudaGetLastError();
+            return fail(h, SU_ENOMEM, "fused schedule upload failed");
+        }
+        it = h->fused.emplace(key, t).first;
+    }
+    *out = &it->second;
+    return SU_OK;
+}
+
+// a dependency wait that gave up (fused_wait) means a broken schedule: report it instead of returning wrong links
+su_status check_fused_error(su_lattice* h) {
+    for (auto& kv : h->fused) {
+        FusedCtrl c{};
+        SU_CUDA(h, cudaMemcpy(&c, kv.second.d_ctrl, sizeof(c), cudaMemcpyDeviceToHost), "fused control read-back");
+        if (c.error) return fail(h, SU_ECUDA, "fused launch: a dependency wait timed out; the links are not valid");
+    }
+    return SU_OK;
+}
+
+// the register kernels of Nc <= 4 can reunitarise the link they have just updated before they store it
+bool reunit_in_kernel(const su_lattice* h) { return !h->var.generic && h->Nc <= 4; }
+
+su_status launch_fused_group(su_lattice* h, double beta, int kind, int pass, int sub0, const uint32_t* d_sweep, bool reunit) {
+    su_lattice::FusedTable* t = nullptr;
+    su_status st = fused_table(h, kind, sub0, &t);
+    if (st != SU_OK) return st;
+    UpdateArgs a{};
+    a.links = h->links; a.g = h->g; a.parity = sub0 >> 2; a.mu = sub0 & 3; a.beta = beta;
+    a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
+    a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = (uint32_t)pass;
+    a.attempts = nullptr; a.counters = h->d_counters; a.reunit = reunit ? 1 : 0;
+    a.fz.work = t->d_work; a.fz.done = t->d_done; a.fz.ctrl = t->d_ctrl; a.fz.fg = t->fg; a.fz.fg.sub0 = sub0;
+    a.fz.n_tickets = t->n_tickets;
+    SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "fused update kernel launch");
+    return SU_OK;
+}
+
 su_status launch_substep(su_lattice* h, double beta, int kind, int pass, int parity, int mu,
-                         uint8_t* d_attempts, const uint32_t* d_sweep) {
+                         uint8_t* d_attempts, const uint32_t* d_sweep, bool reunit = false) {
     UpdateArgs a{};
     a.links = h->links; a.g = h->g; a.parity = parity; a.mu = mu; a.beta = beta;
     a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
     a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = (uint32_t)pass;
-    a.attempts = d_attempts; a.counters = h->d_counters;
+    a.attempts = d_attempts; a.counters = h->d_counters; a.reunit = reunit ? 1 : 0;
     a.peer_lo = h->peer_lo; a.peer_hi = h->peer_hi;
     if (h->g.t_halo && (!h->peer_lo || !h->peer_hi)) return fail(h, SU_ESTATE, "slab lattice: su_slab_set_peers first");
     SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "update kernel launch");
@@ -206,14 +301,30 @@ su_status enqueue_sweep(su_lattice* h, double beta, int n_hb, int n_or, const ui
         ev.n_hb = n_hb; ev.n_or = n_or;
         SU_CUDA(h, cudaEventRecord(ev.e[0], h->stream), "timing event");
     }
+    // "reunit_on_store": every link is updated exactly once in the LAST pass of the sweep; there the Nc <= 4 register
+    // kernels project it back to SU(Nc) before they store it (the other kernels get the reunitarisation kernel below)
+    const bool reunit_store = h->reunit_on_store && h->Nc > 2 - 1 && reunit_in_kernel(h) && n_hb + n_or > 0;
     for (int pass = 0; pass < n_hb + n_or; ++pass) {
         const int kind = pass < n_hb ? KIND_HB : KIND_OR;
+        const bool ru = reunit_store && pass == n_hb + n_or - 1;
         if (timed && pass == n_hb) SU_CUDA(h, cudaEventRecord(ev.e[1], h->stream), "timing event");
-        for (int parity = 0; parity < 2; ++parity)
-            for (int mu = 0; mu < 4; ++mu) {
-                su_status st = launch_substep(h, beta, kind, kind == KIND_HB ? pass : 0, parity, mu, nullptr, d_sweep);
+        const int g = effective_fuse(h, kind);
+        if (g > 1) {
+            for (int sub0 = 0; sub0 < 8; sub0 += g) {        // sub-step index = 4 parity + mu (reading R6)
+                su_status st = launch_fused_group(h, beta, kind, kind == KIND_HB ? pass : 0, sub0, d_sweep, ru);
                 if (st != SU_OK) return st;
             }
+            continue;
+        }
+        for (int parity = 0; parity < 2; ++parity)
+            for (int mu = 0; mu < 4; ++mu) {
+                su_status st = launch_substep(h, beta, kind, kind == KIND_HB ? pass : 0, parity, mu, nullptr, d_sweep, ru);
+                if (st != SU_OK) return st;
+            }
+    }
+    if (h->reunit_on_store && !reunit_store && n_hb + n_or > 0) {
+        AuxArgs ra = aux_args(h);
+        SU_CUDA(h, SU_BY_NC(h, reunit_nc, h->var, ra, h->stream, &h->n_launch), "reunitarise kernel");
     }
     if (timed) {
         if (n_or == 0) SU_CUDA(h, cudaEventRecord(ev.e[1], h->stream), "timing event");
@@ -329,7 +440,8 @@ static su_status create_common(int Nc, int Lx, int Ly, int Lz, int Lt_glob, bool
     }
     const unsigned Vs = (unsigned)Lx * Ly * Lz;
     // partial sums of the reductions: one per block; the row-per-lane kernels have as few as 4 sites per block
-    const size_t npart = (h->var.generic ? 2 * ((size_t)h->g.Vh / ROWS_MIN_LINKS_PER_BLOCK + 1)
+    const size_t npart = Nc > SUG_MAX_TEMPLATE_NC ? 2 * (size_t)h->g.Vh + 2 :
+                         (h->var.generic ? 2 * ((size_t)h->g.Vh / ROWS_MIN_LINKS_PER_BLOCK + 1)
                                          : (size_t)plaquette_blocks(h->g.Vh) + 2 * (size_t)reduce_blocks(Vs)) + 2;
     if (st == SU_OK && cudaMalloc(&h->d_partials, npart * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_result, 2 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
@@ -429,6 +541,7 @@ su_status su_lattice_destroy(su_lattice* h) {
     DeviceGuard guard(h->device);
     cudaStreamSynchronize(h->stream);
     free_graphs(h);
+    free_fused(h);
     drain_timing(h);
     for (cudaEvent_t e : h->free_events) cudaEventDestroy(e);
     if (h->owns_links && h->links) cudaFree(h->links);
@@ -480,6 +593,14 @@ su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
     if (su_status hs = halos_ok(h, "su_sweep")) return hs;
     if (h->graph_mode && h->timing) return fail(h, SU_EUNSUPPORTED, "su_sweep: per-kind timing is not available in graph mode");
     DeviceGuard guard(h->device);
+    for (int kind = 0; kind < 2; ++kind) {           // build the fused tables outside any stream capture
+        if ((kind == KIND_HB ? n_hb : n_or) == 0 || effective_fuse(h, kind) <= 1) continue;
+        for (int sub0 = 0; sub0 < 8; sub0 += h->fuse_g) {
+            su_lattice::FusedTable* t = nullptr;
+            su_status st = fused_table(h, kind, sub0, &t);
+            if (st != SU_OK) return st;
+        }
+    }
     if (!h->graph_mode) {
         su_status st = enqueue_sweep(h, beta, n_hb, n_or, nullptr, h->timing);
         if (st != SU_OK) return st;
@@ -499,6 +620,7 @@ su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
             const uint64_t before = h->n_launch;
             if (e == cudaSuccess) st = enqueue_sweep(h, beta, n_hb, n_or, h->d_sweep, false);
             if (e == cudaSuccess) e = cudaStreamEndCapture(cap, &graph);
+            h->graph_launches[key] = h->n_launch - before;
             h->n_launch = before;
             h->stream = user;
             cudaGraphExec_t exec = nullptr;
@@ -512,7 +634,7 @@ su_status su_sweep(su_lattice* h, double beta, int n_hb, int n_or) {
         k_set_u32<<<1, 1, 0, h->stream>>>(h->d_sweep, h->sweep);
         SU_CUDA(h, cudaGetLastError(), "sweep counter upload");
         SU_CUDA(h, cudaGraphLaunch(it->second, h->stream), "graph launch");
-        h->n_launch += 1 + (uint64_t)(n_hb + n_or) * 8;
+        h->n_launch += 1 + h->graph_launches[key];
     }
     ++h->sweep;
     return SU_OK;
@@ -554,6 +676,7 @@ su_status su_plaquette(su_lattice* h, double* out) {
     double v = 0;
     SU_CUDA(h, cudaMemcpyAsync(&v, h->d_result, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "plaquette copy");
     SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_plaquette synchronise");
+    if (su_status fs = check_fused_error(h)) return fs;
     *out = v;
     return SU_OK;
 }
@@ -634,12 +757,87 @@ su_status su_import_links(su_lattice* h, const double* host_src, size_t n_double
     return st;
 }
 
+// ---- configuration files ("file storing ... configurations") ----
+namespace {
+struct ConfigHeader {          // 64 bytes, little-endian
+    char magic[8];             // "SUGCONF1"
+    int32_t Nc, L[4], precision, storage, reserved;
+    uint64_t seed;
+    uint32_t sweep, pad;
+    double plaquette;          // of the stored configuration, recomputed and compared on load
+};
+static_assert(sizeof(ConfigHeader) == 64, "configuration file header");
+uint64_t fnv1a(const void* p, size_t n, uint64_t h) {
+    const unsigned char* b = (const unsigned char*)p;
+    for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+    return h;
+}
+}  // namespace
+
+su_status su_save_config(su_lattice* h, const char* path) {
+    if (!h || !path) return SU_EINVAL;
+    if (!h->ready) return fail(h, SU_ESTATE, "su_save_config before su_init_* / su_import_links");
+    if (h->g.t_halo) return fail(h, SU_EUNSUPPORTED, "su_save_config: export the slabs and write them from the driver");
+    ConfigHeader hd{};
+    memcpy(hd.magic, "SUGCONF1", 8);
+    hd.Nc = h->Nc; for (int d = 0; d < 4; ++d) hd.L[d] = h->g.L[d];
+    hd.precision = (int)h->prec; hd.storage = h->var.store == STORE_RECON12 ? 1 : 0;
+    hd.seed = h->seed; hd.sweep = h->sweep;
+    su_status st = su_plaquette(h, &hd.plaquette);
+    if (st != SU_OK) return st;
+    const size_t n = h->V * 4 * 2 * (size_t)h->Nc * h->Nc;
+    std::vector<double> buf;
+    try { buf.resize(n); } catch (...) { return fail(h, SU_ENOMEM, "su_save_config: host buffer"); }
+    st = su_export_links(h, buf.data(), n);
+    if (st != SU_OK) return st;
+    FILE* f = fopen(path, "wb");
+    if (!f) return fail(h, SU_EINVAL, "su_save_config: cannot open '%s' for writing", path);
+    const uint64_t sum = fnv1a(buf.data(), n * sizeof(double), fnv1a(&hd, sizeof(hd), 14695981039346656037ull));
+    const bool ok = fwrite(&hd, sizeof(hd), 1, f) == 1 && fwrite(buf.data(), sizeof(double), n, f) == n && fwrite(&sum, 8, 1, f) == 1;
+    if (fclose(f) != 0 || !ok) return fail(h, SU_EINVAL, "su_save_config: write to '%s' failed", path);
+    return SU_OK;
+}
+
+su_status su_load_config(su_lattice* h, const char* path) {
+    if (!h || !path) return SU_EINVAL;
+    if (h->g.t_halo) return fail(h, SU_EUNSUPPORTED, "su_load_config: read the file in the driver and import the slabs");
+    FILE* f = fopen(path, "rb");
+    if (!f) return fail(h, SU_EINVAL, "su_load_config: cannot open '%s'", path);
+    ConfigHeader hd{};
+    const size_t n = h->V * 4 * 2 * (size_t)h->Nc * h->Nc;
+    std::vector<double> buf;
+    uint64_t sum = 0;
+    bool ok = fread(&hd, sizeof(hd), 1, f) == 1 && !memcmp(hd.magic, "SUGCONF1", 8);
+    if (ok && (hd.Nc != h->Nc || hd.L[0] != h->g.L[0] || hd.L[1] != h->g.L[1] || hd.L[2] != h->g.L[2] || hd.L[3] != h->g.L[3])) {
+        fclose(f);
+        return fail(h, SU_EINVAL, "su_load_config: '%s' holds another group or lattice", path);
+    }
+    if (ok) { try { buf.resize(n); } catch (...) { fclose(f); return fail(h, SU_ENOMEM, "su_load_config: host buffer"); } }
+    ok = ok && fread(buf.data(), sizeof(double), n, f) == n && fread(&sum, 8, 1, f) == 1;
+    fclose(f);
+    if (!ok) return fail(h, SU_EINVAL, "su_load_config: '%s' is not a complete configuration file", path);
+    if (sum != fnv1a(buf.data(), n * sizeof(double), fnv1a(&hd, sizeof(hd), 14695981039346656037ull)))
+        return fail(h, SU_EINVAL, "su_load_config: checksum mismatch in '%s'", path);
+    su_status st = su_import_links(h, buf.data(), n);
+    if (st != SU_OK) return st;
+    st = su_set_rng(h, hd.seed, hd.sweep);
+    if (st != SU_OK) return st;
+    // the stored plaquette was measured in the writer's precision and storage; a reader in fp32 / two-row storage rounds the links
+    double plaq = 0;
+    st = su_plaquette(h, &plaq);
+    if (st != SU_OK) return st;
+    const double tol = (h->prec == SU_FP64 && hd.precision == (int)SU_FP64) ? 1e-12 : 1e-5;
+    if (!(std::fabs(plaq - hd.plaquette) <= tol)) return fail(h, SU_EINVAL, "su_load_config: plaquette of '%s' does not match its header", path);
+    return SU_OK;
+}
+
 su_status su_get_counters(su_lattice* h, uint64_t* kp_attempts_total, uint64_t* kp_exhausted) {
     if (!h) return SU_EINVAL;
     DeviceGuard guard(h->device);
     unsigned long long v[2] = {0, 0};
     SU_CUDA(h, cudaMemcpyAsync(v, h->d_counters, sizeof(v), cudaMemcpyDeviceToHost, h->stream), "counter copy");
     SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_get_counters synchronise");
+    if (su_status fs = check_fused_error(h)) return fs;
     if (kp_attempts_total) *kp_attempts_total = v[0];
     if (kp_exhausted) *kp_exhausted = v[1];
     return SU_OK;
@@ -649,7 +847,7 @@ su_status su_synchronize(su_lattice* h) {
     if (!h) return SU_EINVAL;
     DeviceGuard guard(h->device);
     SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_synchronize");
-    return SU_OK;
+    return check_fused_error(h);
 }
 
 su_status su_set_graph_mode(su_lattice* h, int enabled) {
@@ -694,7 +892,31 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
         if (value < 0 || value > h->g.L[2] || (value > 0 && h->g.L[2] % value)) return fail(h, SU_EINVAL, "z_chunk_planes must divide Lz");
         SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
         free_graphs(h);
+        free_fused(h);
         h->g.Zc = value > 0 ? (int)value : traversal_z_chunk(h->g, h->link_bytes);
+        return SU_OK;
+    }
+    if (!strcmp(name, "reunit_on_store")) {
+        if (value != 0 && value != 1) return fail(h, SU_EINVAL, "reunit_on_store must be 0 or 1");
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);
+        h->reunit_on_store = value != 0;
+        return SU_OK;
+    }
+    const bool is_fuse = !strcmp(name, "fuse"), is_chunk = !strcmp(name, "fuse_chunk_planes"), is_margin = !strcmp(name, "fuse_margin"),
+               is_cell = !strcmp(name, "fuse_cell_planes");
+    if (is_fuse || is_chunk || is_margin || is_cell) {
+        if (is_fuse && value != 1 && value != 2 && value != 4 && value != 8) return fail(h, SU_EINVAL, "fuse must be 1, 2, 4 or 8");
+        if ((is_chunk || is_cell) && (value < 0 || value > h->g.L[2] || (value > 0 && h->g.L[2] % value)))
+            return fail(h, SU_EINVAL, "%s must divide Lz", name);
+        if (is_margin && (value < 1 || value > 1000000)) return fail(h, SU_EINVAL, "fuse_margin must be >= 1");
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);
+        free_fused(h);
+        if (is_fuse) h->fuse_g = (int)value;
+        if (is_chunk) h->fuse_chunk_planes = (int)value;
+        if (is_margin) h->fuse_margin = (int)value;
+        if (is_cell) h->fuse_cell_planes = (int)value;
         return SU_OK;
     }
     return fail(h, SU_EINVAL, "su_set_option: unknown option '%s'", name);
@@ -703,6 +925,12 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
 su_status su_get_option(su_lattice* h, const char* name, long long* value) {
     if (!h || !name || !value) return SU_EINVAL;
     if (!strcmp(name, "z_chunk_planes")) { *value = h->g.Zc; return SU_OK; }
+    if (!strcmp(name, "reunit_on_store")) { *value = h->reunit_on_store ? 1 : 0; return SU_OK; }
+    if (!strcmp(name, "fuse")) { *value = h->fuse_g; return SU_OK; }
+    if (!strcmp(name, "fuse_chunk_planes")) { *value = h->fuse_chunk_planes; return SU_OK; }
+    if (!strcmp(name, "fuse_margin")) { *value = h->fuse_margin; return SU_OK; }
+    if (!strcmp(name, "fuse_cell_planes")) { *value = h->fuse_cell_planes; return SU_OK; }
+    if (!strcmp(name, "fuse_effective")) { *value = std::max(effective_fuse(h, 0), effective_fuse(h, 1)); return SU_OK; }
     return fail(h, SU_EINVAL, "su_get_option: unknown option '%s'", name);
 }
 

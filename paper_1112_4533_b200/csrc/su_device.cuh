@@ -118,8 +118,21 @@ template <class T> __device__ __forceinline__ void su3_third_row(cx<T>* m) {   /
 // Load / store flavours: LD_PLAIN = ld.global (read-write data), LD_RO = ld.global.nc (neighbour links,
 // read-only during a sub-step, kept in L1/L2 for re-use), LD_STREAM = ld.global.cs / st.global.cs (the
 // link being updated: touched once per sub-step, so it should not displace re-used lines).
-enum : int { LD_PLAIN = 0, LD_RO = 1, LD_STREAM = 2 };
+// LD_COHERENT = ld.relaxed.gpu (served by L2, never by a stale L1 line): links that another block may have
+// rewritten earlier in the SAME launch (fused multi-sub-step launches, fused_schedule.h).
+enum : int { LD_PLAIN = 0, LD_RO = 1, LD_STREAM = 2, LD_COHERENT = 3 };
+__device__ __forceinline__ double2 ld_coherent(const double2* p) {
+    double2 v;
+    asm volatile("ld.relaxed.gpu.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ float2 ld_coherent(const float2* p) {
+    float2 v;
+    asm volatile("ld.relaxed.gpu.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p) : "memory");
+    return v;
+}
 template <class T, int LD> __device__ __forceinline__ typename V2<T>::type ldg2(const typename V2<T>::type* p) {
+    if (LD == LD_COHERENT) return ld_coherent(p);
     return LD == LD_RO ? __ldg(p) : (LD == LD_STREAM ? __ldcs(p) : *p);
 }
 template <class T, bool STREAM> __device__ __forceinline__ void stg2(typename V2<T>::type* p, typename V2<T>::type v) {
@@ -375,9 +388,26 @@ __device__ __forceinline__ void kp_direction(uint32_t k0, uint32_t k1, uint32_t 
     n[0] = sin_t * cp; n[1] = sin_t * sp; n[2] = cos_t;
 }
 
+// The link-independent part of attempt 0 of a draw: Q = ln r1 + cos^2(2 pi r2) ln r3 and R = r4^2, so that
+// lambda^2 = -Q / (2 alpha) and the attempt is accepted iff R <= 1 - lambda^2 - the same expressions, in the
+// same order and precision, as in the accept loop of kp_draw. A kernel evaluates this for all the subgroups of
+// its link before the staple (with the Philox blocks of the subgroups interleaved, in the shadow of the first
+// loads) and hands it to kp_draw as pre0 = {Q, R} at stride dir_stride; attempts >= 1 (a few percent of the
+// draws) still run the loop.
+template <class T>
+__device__ __forceinline__ void kp_attempt0(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2_base, T& Q, T& R) {
+    uint32_t w[4];
+    philox4x32_10(c0, c1, c2_kind(c2_base, RNG_KP), 0u, k0, k1, w);
+    const T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]), r4 = uniform01<T>(w[3]);
+    const T c = Fn<T>::cos2pi(r2);
+    Q = Fn<T>::log(r1) + c * c * Fn<T>::log(r3);
+    R = r4 * r4;
+}
+
 template <class T>
 __device__ __forceinline__ int kp_draw(unsigned draw_mask, T alpha, T m_inv2a, uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
-                                       uint32_t c2_base, T v[4], const T* dir = nullptr, int dir_stride = 0) {
+                                       uint32_t c2_base, T v[4], const T* dir = nullptr, int dir_stride = 0,
+                                       const T* pre0 = nullptr) {
     const bool drawable = (alpha > (T)0) && Fn<T>::finite(alpha);
     const unsigned converged = __ballot_sync(draw_mask, drawable);
     if (!drawable) return 0;
@@ -387,12 +417,18 @@ __device__ __forceinline__ int kp_draw(unsigned draw_mask, T alpha, T m_inv2a, u
     T a0 = 0;
     int used = 0;
     uint32_t w[4];
+    // attempt 0 precomputed by kp_attempt0 (link-independent part): only the scale by -1/(2 alpha) and the test remain
+    bool from_pre = false;
+    if (pre0) {
+        const T lambda2 = pre0[0] * m_inv2a;
+        if (pre0[dir_stride] <= (T)1 - lambda2) { a0 = (T)1 - (T)2 * lambda2; used = 1; from_pre = true; }
+    }
     // lanes leave the accept loop after different numbers of attempts; without an explicit barrier the
     // compiler lets every exit group run the rest of the draw on its own (ncu: the direction part ran 1.6x
     // per warp). draw_mask = the lanes that call kp_draw for this subgroup, balloted by the caller BEFORE its
     // divergent branch (all of them reach the barrier: the early return above is taken before the loop by
     // lanes that then skip it, so they are excluded here).
-    for (int n = 0; n < KP_MAX_ATTEMPTS; ++n) {
+    for (int n = pre0 ? 1 : 0; !from_pre && n < KP_MAX_ATTEMPTS; ++n) {
         philox4x32_10(c0, c1, c2_kind(c2_base, RNG_KP), (uint32_t)n, k0, k1, w);
         if (PRETEST) {
             const float S = 2.3283064365386963e-10f;      // 2^-32
@@ -410,7 +446,7 @@ __device__ __forceinline__ int kp_draw(unsigned draw_mask, T alpha, T m_inv2a, u
     }
     __syncwarp(converged);
     if (!used) return 0;
-    if (PRETEST) {
+    if (PRETEST && !from_pre) {
         T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]);
         T c = Fn<T>::cos2pi(r2);
         T lambda2 = (Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) * m_inv2a;
@@ -443,7 +479,7 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                                                  uint32_t c0, uint32_t c1, uint32_t c2_base,
                                                  uint8_t* att_out, size_t att_stride,
                                                  unsigned& att_total, unsigned& exhausted, unsigned warp_mask,
-                                                 const T* dirs = nullptr, int dir_stride = 0) {
+                                                 const T* dirs = nullptr, int dir_stride = 0, const T* pre = nullptr) {
     // warp_mask: the lanes of this warp that run the subgroup loop (balloted by the kernel where all of them
     // are converged); every one of them executes the ballots below, subgroup by subgroup
     int q = 0;
@@ -467,7 +503,8 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                     T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                     T v[4];
                     used = kp_draw<T>(draw_mask, two_beta_over_nc * k, m_nc_over_4beta * ik, k0, k1, c0, c1,
-                                      c2_base | (uint32_t)q, v, dirs ? dirs + 3 * q * dir_stride : nullptr, dir_stride);
+                                      c2_base | (uint32_t)q, v, dirs ? dirs + 3 * q * dir_stride : nullptr, dir_stride,
+                                      pre ? pre + 2 * q * dir_stride : nullptr);
                     if (used) quat_mul(v, ud, a); else ok = false;
                 } else {
                     // a = (u~^dagger)^2 = conj(r)^2 / k^2 (eq 17): no square root, one reciprocal
@@ -495,6 +532,90 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                 }
             }
         }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Gram-Schmidt / determinant on a local matrix (rolled loops), used by reunitarise (Nc >= 4)
+// and by the hot start (always double, reading R20).
+// ------------------------------------------------------------------------------------------
+template <int NC, class R, bool UNR = false>
+__device__ __forceinline__ void gram_schmidt_rows(cx<R>* U, int nrows) {
+#pragma unroll(UNR ? NC : 1)
+    for (int r = 0; r < (UNR ? NC : nrows); ++r) {
+#pragma unroll(UNR ? NC : 1)
+        for (int p = 0; p < r; ++p) {
+            cx<R> dot = mk<R>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+            for (int k = 0; k < NC; ++k) mad_ca(dot, U[p * NC + k], U[r * NC + k]);
+#pragma unroll(UNR ? NC : 1)
+            for (int k = 0; k < NC; ++k) U[r * NC + k] = U[r * NC + k] - dot * U[p * NC + k];
+        }
+        R n2 = 0;
+#pragma unroll(UNR ? NC : 1)
+        for (int k = 0; k < NC; ++k) n2 += U[r * NC + k].re * U[r * NC + k].re + U[r * NC + k].im * U[r * NC + k].im;
+        R inv = (R)1 / Fn<R>::sqrt(n2);
+#pragma unroll(UNR ? NC : 1)
+        for (int k = 0; k < NC; ++k) U[r * NC + k] = inv * U[r * NC + k];
+    }
+}
+
+// det of a 4x4 complex matrix by the 2x2-minor (Laplace) expansion over rows {0,1} x {2,3}: no pivoting,
+// no dynamic indexing, so it stays in registers (used for the phase conj(det)/|det| only).
+template <class R>
+__device__ __forceinline__ cx<R> determinant4(const cx<R>* A) {
+    const cx<R> s0 = A[0] * A[5] - A[1] * A[4], s1 = A[0] * A[6] - A[2] * A[4], s2 = A[0] * A[7] - A[3] * A[4];
+    const cx<R> s3 = A[1] * A[6] - A[2] * A[5], s4 = A[1] * A[7] - A[3] * A[5], s5 = A[2] * A[7] - A[3] * A[6];
+    const cx<R> c5 = A[10] * A[15] - A[11] * A[14], c4 = A[9] * A[15] - A[11] * A[13], c3 = A[9] * A[14] - A[10] * A[13];
+    const cx<R> c2 = A[8] * A[15] - A[11] * A[12], c1 = A[8] * A[14] - A[10] * A[12], c0 = A[8] * A[13] - A[9] * A[12];
+    return (s0 * c5 - s1 * c4) + (s2 * c3 + s3 * c2) + (s5 * c0 - s4 * c1);
+}
+
+// SU(3) rows 0,1 by modified Gram-Schmidt in registers (same operation order as gram_schmidt_rows)
+template <class T>
+__device__ __forceinline__ void gram_schmidt_su3_two_rows(cx<T>* U) {
+    T n2 = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) n2 += U[k].re * U[k].re + U[k].im * U[k].im;
+    T inv = (T)1 / Fn<T>::sqrt(n2);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) U[k] = inv * U[k];
+    cx<T> dot = mk<T>(0, 0);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) mad_ca(dot, U[k], U[3 + k]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) U[3 + k] = U[3 + k] - dot * U[k];
+    n2 = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) n2 += U[3 + k].re * U[3 + k].re + U[3 + k].im * U[3 + k].im;
+    inv = (T)1 / Fn<T>::sqrt(n2);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) U[3 + k] = inv * U[3 + k];
+}
+
+// Reunitarisation of one link in registers, Nc <= 4 (reading R10): SU(2) normalise the first row
+// (a0, a1, a2, a3) and rebuild the second, SU(3) Gram-Schmidt on rows 0, 1 + cross product, SU(4) Gram-Schmidt +
+// phase of the determinant on the last row. Used by k_reunit and, on request, by the update kernels right before
+// they store (su_set_option "reunit_on_store").
+template <int NC, class T>
+__device__ __forceinline__ void reunitarize_small(cx<T>* U) {
+    static_assert(NC <= 4, "register-resident reunitarisation is for Nc <= 4");
+    if (NC == 2) {
+        T n = Fn<T>::sqrt((U[0].re * U[0].re + U[0].im * U[0].im) + (U[1].re * U[1].re + U[1].im * U[1].im));
+        U[0] = mk<T>(U[0].re / n, U[0].im / n);
+        U[1] = mk<T>(U[1].re / n, U[1].im / n);
+        U[NC * NC - 2] = mk<T>(-U[1].re, U[1].im);
+        U[NC * NC - 1] = mk<T>(U[0].re, -U[0].im);
+    } else if (NC == 3) {
+        gram_schmidt_su3_two_rows<T>(U);
+        su3_third_row(U);
+    } else {
+        gram_schmidt_rows<NC, T, true>(U, NC);
+        const cx<T> d = determinant4<T>(U);
+        const T inv = (T)1 / Fn<T>::sqrt(d.re * d.re + d.im * d.im);
+        const cx<T> ph = mk<T>(d.re * inv, -d.im * inv);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) U[(NC - 1) * NC + k] = U[(NC - 1) * NC + k] * ph;
     }
 }
 

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/su_gauge.h"
 #include "su_device.cuh"
 #include "update_kernel.cuh"
@@ -29,6 +31,7 @@ struct AuxArgs {
 // Each returns cudaGetLastError() after the launch; n_launch is incremented per kernel launched.
 #define SUG_DECLARE_NC(N)                                                                                   \
     cudaError_t update_nc##N(const Variant&, int kind, const UpdateArgs&, cudaStream_t, uint64_t* n_launch); \
+    int update_spb_nc##N(const Variant&, int kind);                                                          \
     cudaError_t plaquette_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);           \
     cudaError_t polyakov_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);            \
     cudaError_t reunit_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);              \
@@ -44,6 +47,21 @@ SUG_DECLARE_NC(5)
 SUG_DECLARE_NC(6)
 SUG_DECLARE_NC(7)
 SUG_DECLARE_NC(8)
+
+// fused_schedule.cu
+FusedGeom fused_make_geom(int Lx, int Ly, int Lz, int Lt, int spb, int g, int sub0, int U_force);
+bool fused_build_schedule(const FusedGeom& fg, int chunk_units, int margin, std::vector<uint32_t>& work, int& n_tickets);
+
+// big_kernels.cu: the runtime-Nc warp-per-link path (9 <= Nc <= SU_MAX_NC)
+cudaError_t update_nc_big(const Variant&, int kind, const UpdateArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t plaquette_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t polyakov_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t reunit_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t init_cold_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t init_hot_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t export_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+cudaError_t import_nc_big(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);
+constexpr int SUG_MAX_TEMPLATE_NC = 8;    // kernels compiled per Nc up to here; the warp-per-link path above
 
 constexpr int REDUCE_BLOCK = 256;
 inline unsigned reduce_blocks(unsigned n) { return (n + REDUCE_BLOCK - 1) / REDUCE_BLOCK; }

@@ -12,14 +12,34 @@
 // (at t and t-1) before 2 * Zc/Lz time slices of all planes have streamed through L2.
 #pragma once
 #include "su_device.cuh"
+#include "fused_schedule.h"
 
 namespace sug {
 
 #ifndef SUG_TMINUS_STREAM
 #define SUG_TMINUS_STREAM 1
 #endif
-#ifndef SUG_KP_PREDIR
-#define SUG_KP_PREDIR 1
+// heatbath: what the register kernels evaluate ahead of the staple and park in shared memory (one private column
+// per thread): 0 nothing, 1 the directions of the draws, 2 also attempt 0 of every draw (kp_attempt0).
+// Measured at SU(3) 48^4 (profiles/r02b_heatbath.md): fp32 1 is best (-2.7 % against 0); fp64: 0 1.015 ms,
+// 1 1.006 ms, 2 1.118 ms per sub-step - evaluating the fp64 log / cospi chains early lengthens the time to the
+// first loads more than it shortens the tail, so fp64 keeps everything in the subgroup loop.
+#ifndef SUG_KP_PRE_F32
+#define SUG_KP_PRE_F32 1
+#endif
+#ifndef SUG_KP_PRE_F64
+#define SUG_KP_PRE_F64 0
+#endif
+
+// fused launches: how neighbour links are loaded (3 = LD_COHERENT, ld.relaxed.gpu, always served by L2; 0 = LD_PLAIN,
+// ordinary loads, correct because every work item starts behind an acquire at gpu scope, which also invalidates
+// L1) and whether the updated link is stored / the own link loaded with the streaming (evict-first) hint of the
+// plain kernel (there the link is not touched again in the launch; in a fused launch the next stages re-read it)
+#ifndef SUG_FUSED_LD
+#define SUG_FUSED_LD 0
+#endif
+#ifndef SUG_FUSED_STREAM
+#define SUG_FUSED_STREAM 0
 #endif
 
 struct UpdateArgs {
@@ -29,12 +49,21 @@ struct UpdateArgs {
     double beta;
     uint32_t k0, k1, sweep, pass;
     const uint32_t* sweep_ptr;         // device; when non-NULL the sweep counter is read from here (graph replay)
+    int reunit;                        // != 0: project the updated link back to SU(Nc) right before the store (Nc <= 4 register kernels)
     uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
     unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
     // slab mode: link buffers of the slabs below / above in t (peer memory over NVLink, or this device). The
     // kernel that updates a link of the first / last owned slice also stores it into that neighbour's halo.
     void* peer_lo;
     void* peer_hi;
+    // fused launch of several consecutive sub-steps (fused_schedule.h); work == NULL: the plain one-sub-step launch
+    struct Fused {
+        const uint32_t* work;          // device, [n_tickets][g]: tile id (cell * nT + tile) of every stage, or FUSED_NONE
+        unsigned* done;                // device, [g][cells]: cumulative count of finished tiles
+        FusedCtrl* ctrl;               // device
+        FusedGeom fg;
+        unsigned n_tickets;            // = grid size
+    } fz;
 };
 
 // checkerboard index, in the neighbour's buffer, of the halo copy of an edge site (all slabs have Lt_int slices)
@@ -52,17 +81,9 @@ __device__ __forceinline__ int sel4(int i, int v0, int v1, int v2, int v3) {
     return i == 0 ? v0 : (i == 1 ? v1 : (i == 2 ? v2 : v3));
 }
 
-// traversal index (over the OWNED sites of one parity) -> site; all indices stay in registers
-__device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int parity, SiteNbr& s) {
+// (x/2, y, z, stored t) of a site of the given parity -> checkerboard index, RNG site index, neighbour offsets
+__device__ __forceinline__ void site_from_coords(const Geom& g, unsigned xh, unsigned y, unsigned z, unsigned t, int parity, SiteNbr& s) {
     const unsigned row = (unsigned)g.Lxh, pl = row * (unsigned)g.L[1];
-    const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
-    const unsigned zc = tix / span;  unsigned r = tix - zc * span;
-    const unsigned ti = r / grp;     r -= ti * grp;
-    const unsigned zi = r / pl;      r -= zi * pl;
-    const unsigned y = r / row;
-    const unsigned xh = r - y * row;
-    const unsigned z = zc * (unsigned)g.Zc + zi;
-    const unsigned t = ti + (unsigned)g.t_halo;                          // stored time slice
     const int sy = (int)row, sz = (int)pl, st = (int)(pl * (unsigned)g.L[2]);
     const int q = (int)((y + z + t + (unsigned)g.t0g + (unsigned)parity) & 1u);          // x = 2 xh + q
     s.cb = xh + row * (y + (unsigned)g.L[1] * (z + (unsigned)g.L[2] * t));
@@ -81,6 +102,20 @@ __device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int 
     }
 }
 
+// traversal index (over the OWNED sites of one parity) -> site; all indices stay in registers
+__device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int parity, SiteNbr& s) {
+    const unsigned row = (unsigned)g.Lxh, pl = row * (unsigned)g.L[1];
+    const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
+    const unsigned zc = tix / span;  unsigned r = tix - zc * span;
+    const unsigned ti = r / grp;     r -= ti * grp;
+    const unsigned zi = r / pl;      r -= zi * pl;
+    const unsigned y = r / row;
+    const unsigned xh = r - y * row;
+    const unsigned z = zc * (unsigned)g.Zc + zi;
+    const unsigned t = ti + (unsigned)g.t_halo;                          // stored time slice
+    site_from_coords(g, xh, y, z, t, parity, s);
+}
+
 // slab mode: 1 = the thread's site lies in the first owned time slice, 2 = in the last one, 0 otherwise.
 // Recomputed from the traversal index at store time so that nothing stays live across the kernel body.
 __device__ __forceinline__ int slab_edge(const Geom& g, unsigned tix) {
@@ -93,95 +128,229 @@ __device__ __forceinline__ int slab_edge(const Geom& g, unsigned tix) {
 // FUSE3: each staple term S += A B C (three links) is evaluated row by row with all three operands
 // loaded up front (Mat::acc_nnd / acc_dnn): half as many load-wait phases per thread as the
 // two-step form (P = A B; S += P C), for the same registers. KUNR: unroll the loop over nu.
-template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, bool FUSE3 = false, bool KUNR = false>
-__global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
+// LDN: how neighbour links are loaded (LD_RO in a plain launch, LD_COHERENT in a fused one).
+//
+// update_link: staple, W = U S^dagger, subgroup loop and store for ONE link U_mu(x), x = s (rows a1-a6).
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, bool FUSE3, bool KUNR, int LDN, int PRE, bool FUSED>
+__device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, const int mu, const SiteNbr& s, const unsigned tix,
+                                            const unsigned warp_mask, const uint32_t sweep_ctr, T* dir_col,
+                                            unsigned& att_total, unsigned& exhausted) {
     typedef LinkIO<NC, T, STORE, UNR> IO;
     typedef Mat<NC, T, UNR> M;
     typedef cx<T> C;
-    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = tix < a.g.Vh_int;
-    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);      // lanes that run the body (ragged last warp)
-    unsigned att_total = 0, exhausted = 0;
-    if (active) {
-        const int p = a.parity, mu = a.mu;
-        SiteNbr s;
-        site_of_thread(a.g, tix, p, s);
-        const unsigned cb = s.cb;
-        const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
-
-        // heatbath, register kernels: the directions of all subgroup draws are link-independent; evaluate them
-        // now, in the shadow of the first loads, and park them in shared memory (one private column per thread)
-        constexpr int NSUB = NC * (NC - 1) / 2;
-        constexpr bool PREDIR = (KIND == KIND_HB) && UNR && SUG_KP_PREDIR && sizeof(T) == 4;   // fp32 only: measured -2.7 % (fp64: +5 %)
-        __shared__ T dir_sm[PREDIR ? 3 * NSUB : 1][PREDIR ? BLOCK : 1];
-        const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
-        if (PREDIR) {
+    constexpr int NSUB = NC * (NC - 1) / 2;
+    constexpr int LDT = (LDN == LD_RO && SUG_TMINUS_STREAM) ? LD_STREAM : LDN;     // links of the time slice below
+    const unsigned cb = s.cb;
+    const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+    // heatbath, register kernels: the directions of all subgroup draws are link-independent; evaluate them
+    // now, in the shadow of the first loads, and park them in shared memory (one private column per thread)
+    if (PRE >= 1) {
 #pragma unroll
-            for (int q = 0; q < NSUB; ++q) {
-                T n[3];
-                kp_direction<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2((int)a.pass, p, mu, q), n);
-                dir_sm[3 * q][threadIdx.x] = n[0]; dir_sm[3 * q + 1][threadIdx.x] = n[1]; dir_sm[3 * q + 2][threadIdx.x] = n[2];
-            }
+        for (int q = 0; q < NSUB; ++q) {
+            T n[3];
+            kp_direction<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2((int)a.pass, p, mu, q), n);
+            dir_col[(3 * q) * BLOCK] = n[0]; dir_col[(3 * q + 1) * BLOCK] = n[1]; dir_col[(3 * q + 2) * BLOCK] = n[2];
         }
+    }
+    if (PRE >= 2) {
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q) {
+            T Q, R;
+            kp_attempt0<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2((int)a.pass, p, mu, q), Q, R);
+            dir_col[(3 * NSUB + 2 * q) * BLOCK] = Q; dir_col[(3 * NSUB + 2 * q + 1) * BLOCK] = R;
+        }
+    }
 
-        C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
-        M::zero(S);
-        const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
+    C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
+    M::zero(S);
+    const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
 #pragma unroll(KUNR ? 3 : 1)
-        for (int k = 0; k < 3; ++k) {
-            const int nu = k + (k >= mu ? 1 : 0);
-            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
-            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
-            const typename IO::T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
-            const typename IO::T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
-            if (FUSE3) {
-                // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
-                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dpnu, B);
-                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dpmu, P);
-                IO::template load<LD_RO>(pl_nu_s, cb, A);
-                M::acc_nnd(S, A, B, P);
-                // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
-                if (SUG_TMINUS_STREAM && k == 2 && nu == 3) {
-                    // links of the time slice below: with the traversal walking up in t this is their last
-                    // use in the sub-step, so they are fetched evict-first and leave L2 to the slices ahead
-                    IO::template load<LD_STREAM>(pl_mu_o, cb + (unsigned)dmnu, B);
-                    IO::template load<LD_STREAM>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
-                    IO::template load<LD_STREAM>(pl_nu_o, cb + (unsigned)dmnu, A);
-                } else {
-                    IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
-                    IO::template load<LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
-                    IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
-                }
-                M::acc_dnn(S, A, B, P);
+    for (int k = 0; k < 3; ++k) {
+        const int nu = k + (k >= mu ? 1 : 0);
+        const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+        const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+        const typename IO::T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
+        const typename IO::T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
+        if (FUSE3) {
+            // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+            IO::template load<LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
+            IO::template load<LDN>(pl_nu_o, cb + (unsigned)dpmu, P);
+            IO::template load<LDN>(pl_nu_s, cb, A);
+            M::acc_nnd(S, A, B, P);
+            // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
+            if (LDT != LDN && k == 2 && nu == 3) {
+                // links of the time slice below: with the traversal walking up in t this is their last
+                // use in the sub-step, so they are fetched evict-first and leave L2 to the slices ahead
+                IO::template load<LDT>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load<LDT>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load<LDT>(pl_nu_o, cb + (unsigned)dmnu, A);
             } else {
-                // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
-                IO::template load<LD_RO>(pl_nu_s, cb, A);
-                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dpnu, B);
-                M::mul_nn(A, B, P);
-                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dpmu, A);
-                M::acc_nd(S, P, A);
-                // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
-                IO::template load<LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
-                IO::template load<LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
-                M::mul_dn(A, B, P);
-                IO::template load<LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), A);
-                M::acc_nn(S, P, A);
+                IO::template load<LDN>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load<LDN>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load<LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
             }
+            M::acc_dnn(S, A, B, P);
+        } else {
+            // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+            IO::template load<LDN>(pl_nu_s, cb, A);
+            IO::template load<LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
+            M::mul_nn(A, B, P);
+            IO::template load<LDN>(pl_nu_o, cb + (unsigned)dpmu, A);
+            M::acc_nd(S, P, A);
+            // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
+            IO::template load<LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
+            IO::template load<LDN>(pl_mu_o, cb + (unsigned)dmnu, B);
+            M::mul_dn(A, B, P);
+            IO::template load<LDN>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), A);
+            M::acc_nn(S, P, A);
         }
-        typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
-        C* U = A;
-        C* W = B;
-        IO::template load<LD_STREAM>(pl_self, cb, U);
-        M::mul_nd(U, S, W);                                   // W = U S^dagger
-        update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex, sweep_ctr,
-                                           pack_c2((int)a.pass, p, mu, 0),
-                                           a.attempts ? a.attempts + cb : nullptr, (size_t)a.g.Vh,
-                                           att_total, exhausted, warp_mask,
-                                           PREDIR ? &dir_sm[0][threadIdx.x] : nullptr, PREDIR ? BLOCK : 0);
-        IO::template store<true>(pl_self, cb, U);
-        if (const int edge = slab_edge(a.g, tix)) {          // fused halo push (slab mode only)
+    }
+    typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
+    C* U = A;
+    C* W = B;
+    constexpr bool STREAM_SELF = !FUSED || SUG_FUSED_STREAM;
+    IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, U);
+    M::mul_nd(U, S, W);                                   // W = U S^dagger
+    update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex, sweep_ctr,
+                                       pack_c2((int)a.pass, p, mu, 0),
+                                       a.attempts ? a.attempts + cb : nullptr, (size_t)a.g.Vh,
+                                       att_total, exhausted, warp_mask,
+                                       PRE >= 1 ? dir_col : nullptr, PRE >= 1 ? BLOCK : 0,
+                                       PRE >= 2 ? dir_col + 3 * NSUB * BLOCK : nullptr);
+    if (UNR && NC <= 4) {
+        if (a.reunit) reunitarize_small<NC <= 4 ? NC : 2, T>(U);       // su_set_option "reunit_on_store": last pass of a sweep
+    }
+    IO::template store<STREAM_SELF>(pl_self, cb, U);
+    if (!FUSED) {                             // plain launch: halo push fused into the store (slab mode only);
+        if (const int edge = slab_edge(a.g, tix)) {       // recomputed here so that nothing stays live across the body
             if (edge & 1) IO::template store<true>(IO::plane(a.peer_lo, a.g, mu, p), halo_cb_lo(a.g, cb), U);
             if (edge & 2) IO::template store<true>(IO::plane(a.peer_hi, a.g, mu, p), halo_cb_hi(a.g, cb), U);
+        }
+    }
+}
+
+// ---- fused launches: waiting for and signalling the completion of (stage, cell) (fused_schedule.h) ----
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+#ifndef SUG_FUSED_SPIN_LIMIT
+#define SUG_FUSED_SPIN_LIMIT (1u << 20)      // ~0.5 s of polling; a correct schedule never gets near it
+#endif
+// warp 0 of the block, non-blocking: true iff every dependency of the work item is already complete
+__device__ __forceinline__ bool fused_probe(const UpdateArgs::Fused& fz, int s, int cell, int tile, unsigned epoch) {
+    const unsigned target = (epoch + 1u) * (unsigned)fz.fg.nT;
+    bool ok = true;
+    for (int k = (int)threadIdx.x; k < s * FUSED_DEPS_PER_STAGE; k += 32) {
+        const int idx = fused_dep(fz.fg, s, cell, tile, k);
+        if (idx >= 0 && (int)(ld_acquire_u32(fz.done + idx) - target) < 0) ok = false;
+    }
+    return __all_sync(0xffffffffu, ok);
+}
+// warp 0 of the block: every lane polls some of the work item's dependencies
+__device__ __forceinline__ void fused_wait(const UpdateArgs::Fused& fz, int s, int cell, int tile, unsigned epoch) {
+    const unsigned target = (epoch + 1u) * (unsigned)fz.fg.nT;
+    for (int k = (int)threadIdx.x; k < s * FUSED_DEPS_PER_STAGE; k += 32) {
+        const int idx = fused_dep(fz.fg, s, cell, tile, k);
+        if (idx < 0) continue;
+        unsigned spins = 0;
+        while ((int)(ld_acquire_u32(fz.done + idx) - target) < 0) {
+            __nanosleep(64);
+            ++spins;
+            // give up (and make every other block give up at once) rather than hang the device on a broken schedule
+            if ((spins & 255u) == 0 && *(volatile unsigned*)&fz.ctrl->error) break;
+            if (spins > SUG_FUSED_SPIN_LIMIT) { atomicExch(&fz.ctrl->error, 1u); break; }
+        }
+    }
+    __syncwarp();
+}
+
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, bool FUSE3 = false, bool KUNR = false, bool FUSED = false>
+__global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
+    constexpr int NSUB = NC * (NC - 1) / 2;
+    constexpr int PRE = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
+    __shared__ T dir_sm[PRE >= 2 ? 5 * NSUB : (PRE == 1 ? 3 * NSUB : 1)][PRE ? BLOCK : 1];
+    const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
+    unsigned att_total = 0, exhausted = 0;
+    if (!FUSED) {
+        const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
+        const bool active = tix < a.g.Vh_int;
+        const unsigned warp_mask = __ballot_sync(0xffffffffu, active);      // lanes that run the body (ragged last warp)
+        if (active) {
+            SiteNbr s;
+            site_of_thread(a.g, tix, a.parity, s);
+            update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, LD_RO, PRE, false>(
+                a, a.parity, a.mu, s, tix, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
+        }
+    } else {
+        __shared__ unsigned sh_ticket, sh_epoch, sh_ready[2];     // sh_ready alternates per phase: no reuse race
+        if (threadIdx.x == 0) {
+            sh_epoch = *(volatile unsigned*)&a.fz.ctrl->epoch;
+            sh_ticket = atomicAdd(&a.fz.ctrl->ticket, 1u);
+        }
+        __syncthreads();
+        const unsigned ticket = sh_ticket, epoch = sh_epoch;
+        const int ncells = a.fz.fg.Lt * a.fz.fg.nzu, g = a.fz.fg.g;
+        const uint32_t* work = a.fz.work + (size_t)ticket * g;
+        // Phase boundary = normally ONE block barrier. Warp 0 PROBES the dependencies of the next work item as soon as
+        // it has issued its own stores of the current one (the other warps are still computing); after the barrier
+        // the last warp publishes the finished item (fence + counter) while everybody already loads for the next
+        // one. Only if the probe failed does warp 0 spin, after the publication (publishing must never wait on other
+        // blocks: that would chain the blocks' signals one behind the other), followed by a second barrier.
+        int st = 0, flip = 0;
+        while (st < g && __ldg(work + st) == FUSED_NONE) ++st;
+        if (st > 0 && st < g) {                                // a block whose first item is not of stage 0 (pipeline drain)
+            const uint32_t id = __ldg(work + st);
+            const int cell = (int)(id / (unsigned)a.fz.fg.nT);
+            if (threadIdx.x < 32) fused_wait(a.fz, st, cell, (int)(id - (unsigned)cell * (unsigned)a.fz.fg.nT), epoch);
+            __syncthreads();
+        }
+#pragma unroll 1
+        while (st < g) {
+            const uint32_t id = __ldg(work + st);              // uniform over the block
+            const int cell = (int)(id / (unsigned)a.fz.fg.nT), tile = (int)(id - (unsigned)cell * (unsigned)a.fz.fg.nT);
+            const unsigned r = (unsigned)tile * BLOCK + threadIdx.x;
+            const bool active = r < (unsigned)a.fz.fg.cell_sites;
+            const unsigned warp_mask = __ballot_sync(0xffffffffu, active);
+            if (active) {
+                const unsigned t = (unsigned)cell / (unsigned)a.fz.fg.nzu, zu = (unsigned)cell - t * (unsigned)a.fz.fg.nzu;
+                const unsigned zi = r / (unsigned)a.fz.fg.plane_sites, rem = r - zi * (unsigned)a.fz.fg.plane_sites;
+                const unsigned y = rem / (unsigned)a.g.Lxh, xh = rem - y * (unsigned)a.g.Lxh;
+                const int p = fused_parity(a.fz.fg, st), mu = fused_mu(a.fz.fg, st);
+                SiteNbr s;
+                site_from_coords(a.g, xh, y, zu * (unsigned)a.fz.fg.U + zi, t, p, s);
+                update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, SUG_FUSED_LD, PRE, true>(
+                    a, p, mu, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
+            }
+            int nx = st + 1;
+            while (nx < g && __ldg(work + nx) == FUSED_NONE) ++nx;
+            uint32_t idn = 0;
+            int celln = 0, tilen = 0;
+            if (nx < g) {
+                idn = __ldg(work + nx);
+                celln = (int)(idn / (unsigned)a.fz.fg.nT); tilen = (int)(idn - (unsigned)celln * (unsigned)a.fz.fg.nT);
+                if (threadIdx.x < 32) {
+                    const bool ok = fused_probe(a.fz, nx, celln, tilen, epoch);
+                    if (threadIdx.x == 0) sh_ready[flip] = ok ? 1u : 0u;
+                }
+            }
+            if (st + 1 < g) {                                  // nobody waits for the last stage
+                __syncthreads();
+                if (threadIdx.x == BLOCK - 32) { __threadfence(); atomicAdd(a.fz.done + (size_t)st * ncells + cell, 1u); }
+                if (nx < g && !sh_ready[flip]) {               // uniform: written before the barrier
+                    if (threadIdx.x < 32) fused_wait(a.fz, nx, celln, tilen, epoch);
+                    __syncthreads();
+                }
+            }
+            st = nx; flip ^= 1;
+        }
+        if (threadIdx.x == 0) {                                // the last block out re-arms the table for the next launch
+            if (atomicAdd(&a.fz.ctrl->exited, 1u) == a.fz.n_tickets - 1u) {
+                a.fz.ctrl->ticket = 0; a.fz.ctrl->exited = 0;
+                __threadfence();
+                a.fz.ctrl->epoch = epoch + 1u;
+            }
         }
     }
     if (KIND == KIND_HB) {
@@ -278,6 +447,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
         }
         if (ok) {
             quat_mul(a4, U, P);
+            if (a.reunit) {
+                const T inv = (T)1 / Fn<T>::sqrt(P[0] * P[0] + P[1] * P[1] + P[2] * P[2] + P[3] * P[3]);
+                P[0] *= inv; P[1] *= inv; P[2] *= inv; P[3] *= inv;
+            }
             T2* q = pl_self + qsite<T>(cb);
             stg2<T, true>(q, V2<T>::make(P[0], P[1]));
             stg2<T, true>(q + LINK_TILE, V2<T>::make(P[2], P[3]));

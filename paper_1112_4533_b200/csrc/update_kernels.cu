@@ -20,25 +20,36 @@ template <int BLOCK_, int MINB_, bool FUSE3_ = false, bool KUNR_ = false> struct
     static constexpr bool FUSE3 = FUSE3_, KUNR = KUNR_;
 };
 
+// a.fz.work != NULL: the fused launch of a.fz.fg.g consecutive sub-steps (fused_schedule.h), one block per ticket
 template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB>
 static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t st) {
+    const bool fused = a.fz.work != nullptr;
     if (kind == KIND_HB) {
         const unsigned grid = (a.g.Vh_int + HB::BLOCK - 1) / HB::BLOCK;
-        k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR><<<grid, HB::BLOCK, 0, st>>>(a);
+        if (fused) k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR, true><<<a.fz.n_tickets, HB::BLOCK, 0, st>>>(a);
+        else       k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR><<<grid, HB::BLOCK, 0, st>>>(a);
     } else {
         const unsigned grid = (a.g.Vh_int + OR::BLOCK - 1) / OR::BLOCK;
-        k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR><<<grid, OR::BLOCK, 0, st>>>(a);
+        if (fused) k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR, true><<<a.fz.n_tickets, OR::BLOCK, 0, st>>>(a);
+        else       k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR><<<grid, OR::BLOCK, 0, st>>>(a);
     }
     return cudaGetLastError();
 }
+template <class HB, class OR = HB> static int spb_t(int kind) { return kind == KIND_HB ? HB::BLOCK : OR::BLOCK; }
 
 // Tuning overrides (-DSUG_CFG_...="Cfg<...>"), used only while sweeping on the GPU; the defaults below are
 // the measured choices (profiles/).
+#ifndef SUG_SU3_F64_BLOCK          // integer knobs: nvcc splits -D values at commas, so Cfg<...> cannot come from the command line
+#define SUG_SU3_F64_BLOCK 128
+#endif
+#ifndef SUG_SU3_F64_MINB
+#define SUG_SU3_F64_MINB 3
+#endif
 #ifndef SUG_CFG_SU3_F64_HB
-#define SUG_CFG_SU3_F64_HB Cfg<128, 3, true, true>
+#define SUG_CFG_SU3_F64_HB Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, true, true>
 #endif
 #ifndef SUG_CFG_SU3_F64_OR
-#define SUG_CFG_SU3_F64_OR Cfg<128, 3, true, true>
+#define SUG_CFG_SU3_F64_OR Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, true, true>
 #endif
 #ifndef SUG_CFG_SU3_F32_HB
 #define SUG_CFG_SU3_F32_HB Cfg<128, 4, true, true>
@@ -107,6 +118,29 @@ cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateA
     return f64 ? launch_update_rows<NC, double>(kind, a, st) : launch_update_rows<NC, float>(kind, a, st);
 #else
     return f64 ? launch_update_rows<NC, double>(kind, a, st) : launch_update_rows<NC, float>(kind, a, st);
+#endif
+}
+
+// Sites per block of the kernel update_nc would launch for this variant and kind = the tile size of the fused
+// schedule; 0: this kernel has no fused form (the caller then runs the sub-steps one launch each).
+int SUG_CAT(update_spb_nc, SUG_NC)(const Variant& v, int kind) {
+    const bool f64 = v.prec == SU_FP64;
+#if SUG_NC == 2
+    if (!v.generic) return 0;
+    return spb_t<GenericCfg>(kind);
+#elif SUG_NC == 3
+    if (!v.generic) {
+        if (v.store == STORE_RECON12) return f64 ? spb_t<SUG_CFG_SU3R_F64_HB, SUG_CFG_SU3R_F64_OR>(kind) : spb_t<SUG_CFG_SU3R_F32_HB, SUG_CFG_SU3R_F32_OR>(kind);
+        return f64 ? spb_t<SUG_CFG_SU3_F64_HB, SUG_CFG_SU3_F64_OR>(kind) : spb_t<SUG_CFG_SU3_F32_HB, SUG_CFG_SU3_F32_OR>(kind);
+    }
+    if (v.store == STORE_RECON12) return spb_t<GenericCfg>(kind);
+    return 0;
+#elif SUG_NC == 4
+    if (!v.generic) return f64 ? spb_t<SUG_CFG_SU4_F64_HB, SUG_CFG_SU4_F64_OR>(kind) : spb_t<SUG_CFG_SU4_F32_HB, SUG_CFG_SU4_F32_OR>(kind);
+    return 0;
+#else
+    (void)f64;
+    return 0;
 #endif
 }
 

@@ -174,17 +174,20 @@ def test_thermalised_means_agree_statistically(mods, Nc, L, beta):
 def test_su3_48_whole_sweep_every_link(mods):
     """P-sweep at full size: one whole su_sweep(1, 4) = 40 kernels at 48^4 fp64 (the z-chunked traversal, the
     launch configuration bench.py times) against the oracle's sweep, all 21 M links at 1e-11, from links the
-    ORACLE has thermalised (3 sweeps of 1 HB + 4 OR from the hot start, ~10 s each on the box's cores)."""
+    ORACLE has thermalised (6 sweeps of 1 HB + 4 OR from the hot start, ~10 s each on the box's cores; after 3 the
+    worst of the 190 M elements was still at 1.7e-11: the tail of the rounding amplification grows with the volume,
+    SURVEY.md 8(c) P-sweep)."""
     su, oracle = mods
     dims = (L_FULL,) * 4
     O = oracle.OracleLattice(3, dims, "fp64")
     O.init_hot(SEED)
-    for _ in range(3):
+    n_therm = 6
+    for _ in range(n_therm):
         O.sweep(BETA, 1, 4)
     G = su.Lattice(3, dims, "fp64")
     assert G.get_option("z_chunk_planes") < L_FULL          # the chunked traversal is what runs here
     G.import_links(O.export_links())
-    G.set_rng(SEED, 3)
+    G.set_rng(SEED, n_therm)
     att0 = O.counters()[0]
     G.sweep(BETA, 1, 4)
     O.sweep(BETA, 1, 4)
