@@ -334,7 +334,9 @@ def run_nc_scan(args, torch, su, local):
     rows = []
     for L in (8, 16):
         for precision in ("fp32", "fp64"):
-            for Nc in range(2, su.SU_MAX_NC + 1):
+            # the paper's range: Nc <= 32 in single, <= 16 in double precision at 8^4; 16^4 up to Nc = 8
+            nc_max = 8 if L == 16 else (32 if precision == "fp32" else 16)
+            for Nc in range(2, nc_max + 1):
                 for kernel in (("specialised", "generic") if Nc <= 4 else ("generic",)):
                     lat = su.Lattice(Nc, (L,) * 4, precision, kernel=kernel, device=local, graph=True)
                     lat.init_cold(1)

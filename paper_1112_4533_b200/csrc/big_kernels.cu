@@ -23,7 +23,7 @@ namespace sug {
 
 namespace {
 
-constexpr int BIG_CW = 8;                 // columns per lane and product chunk
+constexpr int BIG_CW = 8;                 // at most this many columns per lane and product chunk (accumulators in registers)
 
 template <class T> struct BigLink {
     typedef typename V2<T>::type T2;
@@ -41,15 +41,18 @@ template <class T> struct BigLink {
 };
 
 // D (+)= X' Y', X' = X or X^dagger, Y' = Y or Y^dagger; all n x n row-major in shared memory, D distinct from X, Y.
-// Lane -> (row = lane % n, group = lane / n); the 8-column chunks are dealt round-robin to the 32 / n groups.
+// Lane -> (row = lane % n, group = lane / n); the columns are cut into chunks of cw = min(8, ceil(n / groups)) and the
+// chunks dealt round-robin to the 32 / n groups (n = 9: 3 groups x 3 columns, n = 16: 2 x 8, n >= 17: one group, 8 at a time).
 template <class T, bool XD, bool YD, bool ACC>
 __device__ __forceinline__ void wmm(int n, const cx<T>* X, const cx<T>* Y, cx<T>* D, int lane) {
     const int ngroups = 32 / n > 0 ? 32 / n : 1;
     const int row = lane % n, grp = lane / n;
+    const int per_group = (n + ngroups - 1) / ngroups, cw = per_group < BIG_CW ? per_group : BIG_CW;
     if (grp < ngroups && lane < 32) {
         int chunk = 0;
-        for (int c0 = 0; c0 < n; c0 += BIG_CW, ++chunk) {
+        for (int c0 = 0; c0 < n; c0 += cw, ++chunk) {
             if (chunk % ngroups != grp) continue;
+            const int cend = c0 + cw < n ? c0 + cw : n;
             cx<T> acc[BIG_CW];
 #pragma unroll
             for (int jj = 0; jj < BIG_CW; ++jj) acc[jj] = mk<T>(0, 0);
@@ -58,7 +61,7 @@ __device__ __forceinline__ void wmm(int n, const cx<T>* X, const cx<T>* Y, cx<T>
 #pragma unroll
                 for (int jj = 0; jj < BIG_CW; ++jj) {
                     const int col = c0 + jj;
-                    if (col < n) {
+                    if (col < cend) {
                         const cx<T> y = YD ? conj(Y[col * n + k]) : Y[k * n + col];
                         mad(acc[jj], x, y);
                     }
@@ -67,7 +70,7 @@ __device__ __forceinline__ void wmm(int n, const cx<T>* X, const cx<T>* Y, cx<T>
 #pragma unroll
             for (int jj = 0; jj < BIG_CW; ++jj) {
                 const int col = c0 + jj;
-                if (col < n) D[row * n + col] = ACC ? D[row * n + col] + acc[jj] : acc[jj];
+                if (col < cend) D[row * n + col] = ACC ? D[row * n + col] + acc[jj] : acc[jj];
             }
         }
     }

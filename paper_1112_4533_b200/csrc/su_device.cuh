@@ -5,6 +5,15 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+// -DSUG_CHECK=1 (a debug build: SUG_BUILD_VARIANT=check SUG_NVCC_EXTRA=-DSUG_CHECK=1): device-side asserts on every
+// checkerboard index the kernels form (site, 8 neighbours, diagonal neighbour, halo copies) - the bounds check of
+// our own that stands in for compute-sanitizer memcheck, which is closed on this pool (profiles/r02_sanitizers.md).
+#if defined(SUG_CHECK) && SUG_CHECK
+#include <cassert>
+#define SUG_ASSERT(x) assert(x)
+#else
+#define SUG_ASSERT(x) ((void)0)
+#endif
 
 namespace sug {
 
@@ -83,6 +92,7 @@ __device__ __forceinline__ void decode_cb(const Geom& g, unsigned cb, int parity
     c[0] = 2 * (int)xh + ((c[1] + c[2] + c[3] + g.t0g + parity) & 1);
 }
 __device__ __forceinline__ unsigned cb_of(const Geom& g, int x, int y, int z, int t) {
+    SUG_ASSERT(x >= 0 && x < g.L[0] && y >= 0 && y < g.L[1] && z >= 0 && z < g.L[2] && t >= 0 && t < g.L[3]);
     return (unsigned)(x >> 1) + (unsigned)g.Lxh * ((unsigned)y + (unsigned)g.L[1] * ((unsigned)z + (unsigned)g.L[2] * (unsigned)t));
 }
 // lexicographic index of a stored site in the GLOBAL lattice (the RNG counter word c0)

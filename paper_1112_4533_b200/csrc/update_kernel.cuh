@@ -67,8 +67,8 @@ struct UpdateArgs {
 };
 
 // checkerboard index, in the neighbour's buffer, of the halo copy of an edge site (all slabs have Lt_int slices)
-__device__ __forceinline__ unsigned halo_cb_lo(const Geom& g, unsigned cb) { return cb + (unsigned)g.Lt_int * g.Vsh; }   // -> their upper halo
-__device__ __forceinline__ unsigned halo_cb_hi(const Geom& g, unsigned cb) { return cb - (unsigned)g.Lt_int * g.Vsh; }   // -> their lower halo
+__device__ __forceinline__ unsigned halo_cb_lo(const Geom& g, unsigned cb) { SUG_ASSERT(cb + (unsigned)g.Lt_int * g.Vsh < g.Vh); return cb + (unsigned)g.Lt_int * g.Vsh; }   // -> their upper halo
+__device__ __forceinline__ unsigned halo_cb_hi(const Geom& g, unsigned cb) { SUG_ASSERT(cb >= (unsigned)g.Lt_int * g.Vsh); return cb - (unsigned)g.Lt_int * g.Vsh; }   // -> their lower halo
 
 // The site a thread works on and the checkerboard-index offsets of its 8 neighbours.
 struct SiteNbr {
@@ -100,6 +100,13 @@ __device__ __forceinline__ void site_from_coords(const Geom& g, unsigned xh, uns
         s.dp[3] = ((int)t + 1 == g.L[3]) ? -(g.L[3] - 1) * st : st;
         s.dm[3] = (t == 0) ? (g.L[3] - 1) * st : -st;
     }
+#if defined(SUG_CHECK) && SUG_CHECK
+    SUG_ASSERT(s.cb < g.Vh);
+    for (int d = 0; d < 4; ++d) {
+        SUG_ASSERT(s.cb + (unsigned)s.dp[d] < g.Vh && s.cb + (unsigned)s.dm[d] < g.Vh);
+        for (int e = 0; e < 4; ++e) SUG_ASSERT(e == d || s.cb + (unsigned)(s.dm[d] + s.dp[e]) < g.Vh);      // x - d + e
+    }
+#endif
 }
 
 // traversal index (over the OWNED sites of one parity) -> site; all indices stay in registers
