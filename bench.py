@@ -159,6 +159,8 @@ def make_lattice(su, wl, precision, recon12, kernel, rank, device):
     lat = su.Lattice(wl["Nc"], (wl["L"],) * 4, precision, recon12=recon12, kernel=kernel, device=device)
     for k, v in OPTIONS.items():
         lat.set_option(k, v)
+    if wl["Nc"] > 2 and REUNIT_MODE == "on-store":
+        lat.set_option("reunit_on_store", 1)
     if wl["start"] == "hot":
         lat.init_hot(rank_seed(wl, rank))
     else:
@@ -166,10 +168,14 @@ def make_lattice(su, wl, precision, recon12, kernel, rank, device):
     return lat
 
 
+REUNIT_MODE = "on-store"      # --reunit: "on-store" (su_set_option reunit_on_store: inside the sweep's last pass) or "separate"
+
+
 def one_step(lat, beta, reunit):
-    """the whole hot path once: 40 update kernels + reunitarise + both reductions (24 bytes D2H)"""
+    """the whole hot path once: 40 update sub-steps, reunitarisation (Nc >= 3: in the last pass of the sweep where the
+    kernels can do it on store, else / with --reunit separate by su_reunitarize), both reductions (24 bytes D2H)"""
     lat.sweep(beta, N_HB, N_OR)
-    if reunit:
+    if reunit and REUNIT_MODE == "separate":
         lat.reunitarize()
     return lat.plaquette(), lat.polyakov()
 
@@ -597,6 +603,9 @@ def main():
                          "overrelaxation + reunitarise + plaquette) vs Nc at 8^4 and 16^4, beta 6.2, generic and specialised")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE",
                     help="su_set_option knob for every lattice of the run (e.g. fuse=2); recorded in config.options")
+    ap.add_argument("--reunit", default="on-store", choices=["on-store", "separate"],
+                    help="Nc >= 3 reunitarise once per step: inside the sweep's last pass (su_set_option reunit_on_store; the "
+                         "default) or by a separate su_reunitarize call")
     ap.add_argument("--config-table", action="store_true",
                     help="run the five BASELINE.json configs as stated there (sweep counts, histories), GPU and oracle side by "
                          "side; JSON lines plus a markdown table (BASELINE.md section 3). --workload X restricts it to one config")
@@ -606,6 +615,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
     wl = WORKLOADS[args.workload]
+    global REUNIT_MODE
+    REUNIT_MODE = args.reunit
     for kv in args.option:
         k, v = kv.split("=", 1)
         OPTIONS[k] = int(v)
@@ -688,8 +699,9 @@ def main():
                 "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32", "data": "synthetic",
                 "config": {"workload": args.workload, "Nc": wl["Nc"], "lattice": f"{wl['L']}^4", "beta": wl["beta"],
                            "start": f"{wl['start']} (Philox seed {wl['seed']} + rank)", "sweep": "1 heatbath + 4 overrelaxation",
-                           "step": "su_sweep(1,4) + su_reunitarize + su_plaquette + su_polyakov" if wl["Nc"] > 2
-                                   else "su_sweep(1,4) + su_plaquette + su_polyakov",
+                           "step": ("su_sweep(1,4) + su_reunitarize + su_plaquette + su_polyakov" if REUNIT_MODE == "separate"
+                                    else "su_sweep(1,4) with reunitarisation in its last pass (reunit_on_store) + su_plaquette + su_polyakov")
+                                   if wl["Nc"] > 2 else "su_sweep(1,4) + su_plaquette + su_polyakov",
                            "storage": args.storage, "kernel": args.kernel, "options": dict(OPTIONS), "library": su.LIB_PATH,
                            "graph_replay": bool(res.get("graph")),
                            "lattice_bytes": su.lattice_bytes(wl["Nc"], (wl["L"],) * 4, args.precision, recon12),
