@@ -41,13 +41,14 @@ template <class T> struct BigLink {
 };
 
 // D (+)= X' Y', X' = X or X^dagger, Y' = Y or Y^dagger; all n x n row-major in shared memory, D distinct from X, Y.
-// Lane -> (row = lane % n, group = lane / n); the columns are cut into chunks of cw = min(8, ceil(n / groups)) and the
-// chunks dealt round-robin to the 32 / n groups (n = 9: 3 groups x 3 columns, n = 16: 2 x 8, n >= 17: one group, 8 at a time).
+// Lane -> (row = lane % n, group = lane / n); the 8-column chunks are dealt round-robin to the 32 / n groups.
 template <class T, bool XD, bool YD, bool ACC>
 __device__ __forceinline__ void wmm(int n, const cx<T>* X, const cx<T>* Y, cx<T>* D, int lane) {
     const int ngroups = 32 / n > 0 ? 32 / n : 1;
     const int row = lane % n, grp = lane / n;
-    const int per_group = (n + ngroups - 1) / ngroups, cw = per_group < BIG_CW ? per_group : BIG_CW;
+    // (dealing ceil(n / groups) columns to every group instead of chunks of 8 balances the lanes on paper but measured
+    //  slower at Nc = 9, 10 and equal elsewhere: the short chunks lose the reuse of the row element; profiles/r02f)
+    const int cw = BIG_CW;
     if (grp < ngroups && lane < 32) {
         int chunk = 0;
         for (int c0 = 0; c0 < n; c0 += cw, ++chunk) {
