@@ -519,6 +519,34 @@ def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
     clocks = sampler.stop(t0, t1)
     launches = D.lat.launch_count() - n0
     updates_step = (N_HB + N_OR) * 4 * wl["L"] ** 4                  # the whole lattice, once
+    # per-kind sub-step times of THIS rank's slab (two more sweeps, events at the heatbath / overrelaxation boundary)
+    from paper_1112_4533_b200.slab import schedule
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    hb_ms = or_ms = 0.0
+    for _ in range(2):
+        evs[0].record(D.lat.stream)
+        for i, (kind, pass_, parity, mu) in enumerate(schedule(N_HB, N_OR)):
+            if i == 8 * N_HB:
+                evs[1].record(D.lat.stream)
+            D.lat.substep(wl["beta"], kind, pass_, parity, mu)
+            D._order()
+        evs[2].record(D.lat.stream)
+        torch.cuda.synchronize()
+        hb_ms += evs[0].elapsed_time(evs[1]) / (8 * N_HB) / 2
+        or_ms += evs[1].elapsed_time(evs[2]) / (8 * N_OR) / 2
+        D.sweep_counter += 1
+        D.lat.set_rng(D.seed, D.sweep_counter)
+    V_loc = wl["L"] ** 4 // world
+    bpu = algorithmic_bytes_per_update(wl["Nc"], args.precision, recon12)
+    ach = bpu * (V_loc // 2) / (or_ms * 1e-3) / 1e9
+    tf = flops_per_update(wl["Nc"], "or", recon12) * (V_loc // 2) / (or_ms * 1e-3) / 1e12
+    peak = measured_peaks()
+    roof = {"bound": "hbm", "kernel": "staple + overrelaxation update of one slab, one (parity, mu) sub-step incl. the rank ordering (rank 0)",
+            "achieved": ach, "peak": peak[0], "unit": "GB/s", "frac": ach / peak[0], "peak_source": peak[1],
+            "alu": {"achieved_tflops": tf, "peak_tflops": FMA_PEAKS.get(args.precision),
+                    "frac": tf / FMA_PEAKS[args.precision] if FMA_PEAKS.get(args.precision) else None},
+            "avg_launch_ms": or_ms, "hb_avg_launch_ms": hb_ms, "bytes_per_link_update": bpu,
+            "algorithmic_bytes_per_launch": bpu * (V_loc // 2), "traffic": None}
     if rank == 0:
         line = {"metric": METRIC, "value": whole_job_rate(1, updates_step, ms, args.steps), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -531,7 +559,7 @@ def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
                            "parallelism": f"{world} t-slabs of {wl['L'] // world} time slices, halo push fused into the "
                                           "update kernel (peer memory), ordering by a 1-element all-reduce",
                            "l2": "inputs larger than L2 (no flush)"},
-                "roofline": None, "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
+                "roofline": roof, "cpu_baseline": None, "e2e": None, "gpu_launches": launches, "clocks": clocks,
                 "plaquette": plaq}
         print(json.dumps(line), flush=True)
     D.close()
