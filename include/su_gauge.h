@@ -210,6 +210,14 @@ int su_fused_dep_debug(int Lx, int Ly, int Lz, int Lt, int sites_per_block, int 
  * device -1 = current. ms (may be NULL): duration of the best launch. Synchronises the device. */
 su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double* ms);
 
+/* Measured L2 -> SM read throughput of the device in GB/s: every thread block streams one 24 MB L2-resident buffer
+ * with 128-bit loads that bypass L1 (4 blocks of 256 threads per SM, 8 loads per thread in flight, best of 5
+ * launches). The staple + update kernel issues 19 link loads per update of which L1 serves < 10 %, so this, not
+ * HBM, is the roof it runs on for 18-real SU(3) (profiles/r02g). device -1 = current.
+ * ms (may be NULL): duration of the best launch; bytes_per_clock (may be NULL): the same throughput per SM clock
+ * cycle (clock64 span of one block), the figure that carries over to a run at another clock. Synchronises the device. */
+su_status su_measure_l2_peak(int device, double* gbs, double* ms, double* bytes_per_clock);
+
 /* Text of the last error on this handle ("" if none); static text if the handle is NULL.
  * Owned by the library, valid until the next call on the handle. */
 const char* su_last_error(const su_lattice*);

@@ -32,7 +32,7 @@ ABI_SYMBOLS = (
     "su_synchronize", "su_set_graph_mode", "su_set_timing", "su_get_timing", "su_get_launch_count", "su_last_error",
     "su_lattice_create_slab", "su_slab_bytes", "su_slab_links", "su_slab_set_peers", "su_slab_halo_push",
     "su_ipc_export", "su_ipc_open", "su_ipc_close", "su_slab_plaquette_sum", "su_set_option", "su_get_option",
-    "su_measure_fma_peak", "su_save_config", "su_load_config", "su_fused_schedule_debug", "su_fused_dep_debug",
+    "su_measure_fma_peak", "su_measure_l2_peak", "su_save_config", "su_load_config", "su_fused_schedule_debug", "su_fused_dep_debug",
 )
 
 
@@ -98,6 +98,7 @@ def lib():
     L.su_save_config.argtypes = [P, C.c_char_p]
     L.su_load_config.argtypes = [P, C.c_char_p]
     L.su_measure_fma_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D)]
+    L.su_measure_l2_peak.argtypes = [I, C.POINTER(D), C.POINTER(D), C.POINTER(D)]
     L.su_set_option.argtypes = [P, C.c_char_p, C.c_longlong]
     L.su_get_option.argtypes = [P, C.c_char_p, C.POINTER(C.c_longlong)]
     for name in ABI_SYMBOLS:
@@ -126,6 +127,15 @@ def measure_fma_peak(precision="fp64", device=-1):
     if st != SU_OK:
         raise SuError(st, "su_measure_fma_peak")
     return t.value, ms.value
+
+
+def measure_l2_peak(device=-1):
+    """-> (GB/s, ms of the best launch, bytes per SM clock) of the device's L2 -> SM read path (su_measure_l2_peak)"""
+    g, ms, bpc = C.c_double(), C.c_double(), C.c_double()
+    st = lib().su_measure_l2_peak(device, C.byref(g), C.byref(ms), C.byref(bpc))
+    if st != SU_OK:
+        raise SuError(st, "su_measure_l2_peak")
+    return g.value, ms.value, bpc.value
 
 
 class Lattice:

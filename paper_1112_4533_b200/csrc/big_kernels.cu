@@ -6,7 +6,7 @@
 // would be 24 more template instances of everything. Here Nc is a kernel ARGUMENT and ONE WARP owns a link:
 //   * the link's matrices live in shared memory (5 buffers of Nc x Nc complex per warp, dynamic shared memory);
 //   * products are spread over the lanes as (row, block of 8 columns): one operand row element is reused for 8
-//     columns, sums run over k ascending (the oracle's order);
+//     columns, sums run over k ascending (the order of the plain definition);
 //   * the subgroup loop runs the lexicographic sequence as a wavefront of 2 Nc - 3 slots (pairs with i + j = t + 1
 //     are disjoint and commute exactly, as in update_rows_kernel.cuh); a pair is handled by 32 / (Nc / 2) lanes, all
 //     of which evaluate the projection and the Kennedy-Pendleton draw (same counter -> same numbers) and share the

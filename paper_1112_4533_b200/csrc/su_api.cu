@@ -46,6 +46,9 @@ struct su_lattice {
     int fuse_chunk_planes = 0;       // z-planes per chunk of the fused traversal (0: the plain kernel's Zc)
     int fuse_margin = 8;             // tickets between a cell's last tile and the first tile that depends on it
     int fuse_cell_planes = 0;        // z-planes per cell (0: chosen by fused_make_geom)
+    int prefetch_slices = 0;         // update kernels: L2 prefetch distance in time slices (0: off)
+    int blocks_per_sm = 0;           // update kernels: cap on the resident blocks per SM (0: whatever fits)
+    int tile_z = 1, tile_t = 1;      // register update kernels: z-planes x time slices per block tile (Geom::Bz, Bt)
     bool reunit_on_store = false;    // su_sweep leaves reunitarised links (in its last pass; see su_set_option)                     // slab mode: false between su_import_links and su_slab_halo_push
     uint64_t seed = 0;
     uint32_t sweep = 0;
@@ -171,6 +174,28 @@ __global__ void __launch_bounds__(256) k_fma_peak(T* out, const T* in, int iters
     if (s == (T)123456789) out[blockIdx.x * blockDim.x + threadIdx.x] = s;     // never true: keeps the chains alive
 }
 
+// L2 -> SM throughput micro-benchmark (su_measure_l2_peak): every block streams the whole L2-resident buffer with
+// 128-bit loads that bypass L1 (ld.global.cg), 8 independent loads per thread in flight; the sum keeps them alive.
+__global__ void __launch_bounds__(256) k_l2_peak(double* out, const double2* __restrict__ buf, size_t n16, int passes) {
+    double acc = 0;
+    const long long c0 = clock64();
+    const size_t stride = (size_t)blockDim.x * 8;
+    for (int p = 0; p < passes; ++p) {
+        // blocks start at different offsets so that the L2 slices are hit evenly at any instant
+        size_t i = ((size_t)blockIdx.x * 40503u * stride + threadIdx.x) % n16;
+        for (size_t done = 0; done < n16; done += stride) {
+            double2 v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) { size_t j = i + (size_t)k * blockDim.x; if (j >= n16) j -= n16; v[k] = __ldcg(buf + j); }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) acc += v[k].x + v[k].y;
+            i += stride; if (i >= n16) i -= n16;
+        }
+    }
+    if (acc == 123456789.0) out[blockIdx.x * blockDim.x + threadIdx.x] = acc;       // never true
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[0] = (double)(clock64() - c0);     // SM clocks of a block that ran start to end
+}
+
 void free_fused(su_lattice* h) {
     for (auto& kv : h->fused) {
         cudaFree(kv.second.d_work); cudaFree(kv.second.d_done); cudaFree(kv.second.d_ctrl);
@@ -241,6 +266,25 @@ su_status check_fused_error(su_lattice* h) {
 // the register kernels of Nc <= 4 can reunitarise the link they have just updated before they store it
 bool reunit_in_kernel(const su_lattice* h) { return !h->var.generic && h->Nc <= 4; }
 
+// "blocks_per_sm" = n: every update launch asks for so much (unused) dynamic shared memory that only n blocks fit an SM
+int occupancy_cap_bytes(const su_lattice* h) {
+    if (h->blocks_per_sm <= 0) return 0;
+    const int per_sm = 227 * 1024, reserve = 1024 + 8 * 1024;     // 1 KB per block is the system's; headroom for static shared memory
+    return per_sm / h->blocks_per_sm - reserve;
+}
+
+// Block tiles (Geom::Bz, Bt, Wb) for the launch of one sub-step, if the register kernel of this variant and kind can
+// take them: whole warps per x-y plane, whole tiles per z-chunk and per owned time range, whole blocks per segment row.
+void set_block_tile(const su_lattice* h, int kind, Geom& g) {
+    g.Bz = g.Bt = 1; g.Wb = 0;
+    const int spb = h->Nc <= 4 && !h->var.generic && h->Nc > 2 ? update_spb(const_cast<su_lattice*>(h), kind) : 0;
+    const int bz = h->tile_z, bt = h->tile_t, pl = g.Lxh * g.L[1];
+    if (bz * bt <= 1 || spb <= 0 || spb % 32 || pl % 32) return;
+    const int wb = spb / 32;
+    if (wb % (bz * bt) || g.Zc % bz || g.Lt_int % bt || (pl / 32) % (wb / (bz * bt))) return;
+    g.Bz = bz; g.Bt = bt; g.Wb = wb;
+}
+
 su_status launch_fused_group(su_lattice* h, double beta, int kind, int pass, int sub0, const uint32_t* d_sweep, bool reunit) {
     su_lattice::FusedTable* t = nullptr;
     su_status st = fused_table(h, kind, sub0, &t);
@@ -250,6 +294,7 @@ su_status launch_fused_group(su_lattice* h, double beta, int kind, int pass, int
     a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
     a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = (uint32_t)pass;
     a.attempts = nullptr; a.counters = h->d_counters; a.reunit = reunit ? 1 : 0;
+    a.pf_slices = h->prefetch_slices; a.dyn_smem = occupancy_cap_bytes(h);
     a.fz.work = t->d_work; a.fz.done = t->d_done; a.fz.ctrl = t->d_ctrl; a.fz.fg = t->fg; a.fz.fg.sub0 = sub0;
     a.fz.n_tickets = t->n_tickets;
     SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "fused update kernel launch");
@@ -264,6 +309,8 @@ su_status launch_substep(su_lattice* h, double beta, int kind, int pass, int par
     a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = (uint32_t)pass;
     a.attempts = d_attempts; a.counters = h->d_counters; a.reunit = reunit ? 1 : 0;
     a.peer_lo = h->peer_lo; a.peer_hi = h->peer_hi;
+    a.pf_slices = h->prefetch_slices; a.dyn_smem = occupancy_cap_bytes(h);
+    set_block_tile(h, kind, a.g);
     if (h->g.t_halo && (!h->peer_lo || !h->peer_hi)) return fail(h, SU_ESTATE, "slab lattice: su_slab_set_peers first");
     SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "update kernel launch");
     return SU_OK;
@@ -903,6 +950,20 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
         h->reunit_on_store = value != 0;
         return SU_OK;
     }
+    if (!strcmp(name, "block_tile_z") || !strcmp(name, "block_tile_t")) {
+        if (value < 1 || value > 8) return fail(h, SU_EINVAL, "%s must be in 1...8", name);
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);
+        (name[11] == 'z' ? h->tile_z : h->tile_t) = (int)value;
+        return SU_OK;
+    }
+    if (!strcmp(name, "prefetch_slices") || !strcmp(name, "blocks_per_sm")) {
+        if (value < 0 || value > 64) return fail(h, SU_EINVAL, "%s must be in 0...64", name);
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);
+        (name[0] == 'p' ? h->prefetch_slices : h->blocks_per_sm) = (int)value;
+        return SU_OK;
+    }
     const bool is_fuse = !strcmp(name, "fuse"), is_chunk = !strcmp(name, "fuse_chunk_planes"), is_margin = !strcmp(name, "fuse_margin"),
                is_cell = !strcmp(name, "fuse_cell_planes");
     if (is_fuse || is_chunk || is_margin || is_cell) {
@@ -926,6 +987,10 @@ su_status su_get_option(su_lattice* h, const char* name, long long* value) {
     if (!h || !name || !value) return SU_EINVAL;
     if (!strcmp(name, "z_chunk_planes")) { *value = h->g.Zc; return SU_OK; }
     if (!strcmp(name, "reunit_on_store")) { *value = h->reunit_on_store ? 1 : 0; return SU_OK; }
+    if (!strcmp(name, "block_tile_z")) { *value = h->tile_z; return SU_OK; }
+    if (!strcmp(name, "block_tile_t")) { *value = h->tile_t; return SU_OK; }
+    if (!strcmp(name, "prefetch_slices")) { *value = h->prefetch_slices; return SU_OK; }
+    if (!strcmp(name, "blocks_per_sm")) { *value = h->blocks_per_sm; return SU_OK; }
     if (!strcmp(name, "fuse")) { *value = h->fuse_g; return SU_OK; }
     if (!strcmp(name, "fuse_chunk_planes")) { *value = h->fuse_chunk_planes; return SU_OK; }
     if (!strcmp(name, "fuse_margin")) { *value = h->fuse_margin; return SU_OK; }
@@ -984,6 +1049,50 @@ su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double
     const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;     // 64 FMAs per iteration per thread
     *tflops = flops / ((double)best * 1e-3) / 1e12;
     if (ms) *ms = best;
+    return SU_OK;
+}
+
+su_status su_measure_l2_peak(int device, double* gbs, double* ms, double* bytes_per_clock) {
+    if (!gbs) return SU_EINVAL;
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return SU_ECUDA;
+    DeviceGuard guard(dev);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SU_ECUDA;
+    const size_t bytes = 24u << 20, n16 = bytes / 16;           // 24 MB: a fifth of L2, far beyond the SMs' L1
+    const int blocks = prop.multiProcessorCount * 4, threads = 256, passes = 1;
+    void *buf = nullptr, *out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    su_status st = SU_OK;
+    if (cudaMalloc(&buf, bytes) != cudaSuccess || cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)) != cudaSuccess ||
+        cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) st = SU_ENOMEM;
+    float best = 0;
+    double clocks = 0;
+    if (st == SU_OK) {
+        cudaMemset(buf, 0, bytes);
+        for (int rep = 0; rep < 6 && st == SU_OK; ++rep) {          // first repetition = warm-up (brings the buffer into L2)
+            cudaEventRecord(e0, 0);
+            k_l2_peak<<<blocks, threads>>>((double*)out, (const double2*)buf, n16, passes);
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { st = SU_ECUDA; break; }
+            float t = 0;
+            cudaEventElapsedTime(&t, e0, e1);
+            if (rep > 0 && (best == 0 || t < best)) {
+                best = t;
+                cudaMemcpy(&clocks, out, sizeof(double), cudaMemcpyDeviceToHost);
+            }
+        }
+    }
+    if (buf) cudaFree(buf);
+    if (out) cudaFree(out);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (st != SU_OK) { cudaGetLastError(); return st; }
+    // every block reads ceil(n16 / (8 * threads)) * 8 * threads elements per pass
+    const double per_block = (double)((n16 + (size_t)threads * 8 - 1) / ((size_t)threads * 8)) * threads * 8 * 16.0 * passes;
+    *gbs = per_block * blocks / ((double)best * 1e-3) / 1e9;
+    if (ms) *ms = best;
+    if (bytes_per_clock) *bytes_per_clock = clocks > 0 ? per_block * blocks / clocks : 0.0;
     return SU_OK;
 }
 

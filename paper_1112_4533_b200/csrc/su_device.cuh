@@ -64,6 +64,11 @@ struct Geom {
     unsigned Vh;    // stored sites per parity
     unsigned Vhp;   // Vh rounded up to a multiple of LINK_TILE = sites per stored plane
     int Zc;         // z-chunk of the update kernel's traversal order (divides Lz)
+    // Block tiles of the register update kernels (su_set_option "block_tile"): the Wb warps
+    // of a thread block work on the SAME 32-site x-y segments of Bz consecutive z-planes x Bt consecutive time slices
+    // (Wb / (Bz Bt) consecutive segments each), so that links two of them need arrive in L1 once. Bz = Bt = 1: off
+    // (a block is Wb consecutive segments of one plane). Only set in the copy a launch hands to k_update.
+    int Bz, Bt, Wb;
     // t-slab decomposition: the handle owns Lt_int time slices of a global lattice of
     // Lt_glob slices and stores one halo slice below and above them (t_halo = 1). Without it: t_halo = 0,
     // Lt_int = L[3] = Lt_glob, t0g = 0 and the t direction wraps periodically inside the buffer.
@@ -184,6 +189,16 @@ template <int NC, class T, int STORE, bool UNR> struct LinkIO {
                 m[e] = mk<T>(v.x, v.y);
             }
             if (STORE == STORE_RECON12) su3_third_row(m);
+        }
+    }
+    // the E stored elements only (two-row storage: rows 0 and 1, no third-row reconstruction)
+    template <int LD>
+    static __device__ __forceinline__ void load_stored(const T2* __restrict__ pl, unsigned cb, cx<T>* m) {
+        pl = site(pl, cb);
+#pragma unroll(UNR ? E : 1)
+        for (int e = 0; e < E; ++e) {
+            T2 v = ldg2<T, LD>(pl + e * LINK_TILE);
+            m[e] = mk<T>(v.x, v.y);
         }
     }
     template <bool STREAM = false>
@@ -318,6 +333,72 @@ template <int NC, class T, bool UNR> struct Mat {
     static __device__ __forceinline__ void zero(C* S) {
 #pragma unroll(UNR ? NC * NC : 1)
         for (int e = 0; e < NC * NC; ++e) S[e] = mk<T>(0, 0);
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// SU(3) staple terms on two-row operands (12-real storage): a product of SU(3) matrices is in SU(3),
+// so only rows 0 and 1 of a three-link product are multiplied out and its third row is the conjugate cross
+// product of those, exactly as for a stored link. An operand's third row is rebuilt only where the product sums
+// over it. Per term: 2 x 72 multiply-adds + 3 (upper) or 4 (lower) third rows of 24, against 216 + 3 x 24 when
+// every loaded link is completed first.
+// ------------------------------------------------------------------------------------------
+template <class T> struct Su3Rows {
+    typedef cx<T> C;
+    // S += (A B) C^dagger, A: rows 0,1; B, C: rows 0,1 stored, row 2 rebuilt here (B[6..8], C[6..8] are scratch)
+    static __device__ __forceinline__ void acc_upper(C* S, const C* A, C* B, C* D) {
+        su3_third_row(B);
+        su3_third_row(D);
+        C P[9];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            C r[3];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) mad(s, A[i * 3 + k], B[k * 3 + j]);
+                r[j] = s;
+            }
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) mad_cb(s, r[k], D[j * 3 + k]);
+                P[i * 3 + j] = s;
+            }
+        }
+        su3_third_row(P);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) S[e] = S[e] + P[e];
+    }
+    // S += (A^dagger B) C, all three operands: rows 0,1 stored, row 2 rebuilt here
+    static __device__ __forceinline__ void acc_lower(C* S, C* A, C* B, C* D) {
+        su3_third_row(A);
+        su3_third_row(B);
+        su3_third_row(D);
+        C P[9];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            C r[3];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) mad_ca(s, A[k * 3 + i], B[k * 3 + j]);
+                r[j] = s;
+            }
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                C s = mk<T>(0, 0);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) mad(s, r[k], D[k * 3 + j]);
+                P[i * 3 + j] = s;
+            }
+        }
+        su3_third_row(P);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) S[e] = S[e] + P[e];
     }
 };
 

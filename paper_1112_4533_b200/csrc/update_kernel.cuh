@@ -50,6 +50,8 @@ struct UpdateArgs {
     uint32_t k0, k1, sweep, pass;
     const uint32_t* sweep_ptr;         // device; when non-NULL the sweep counter is read from here (graph replay)
     int reunit;                        // != 0: project the updated link back to SU(Nc) right before the store (Nc <= 4 register kernels)
+    int pf_slices;                     // > 0: every warp asks L2 for the link tiles of its sites' positions this many time slices ahead
+    int dyn_smem;                      // host side only: unused dynamic shared memory per block (caps the resident blocks per SM)
     uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
     unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
     // slab mode: link buffers of the slabs below / above in t (peer memory over NVLink, or this device). The
@@ -109,27 +111,68 @@ __device__ __forceinline__ void site_from_coords(const Geom& g, unsigned xh, uns
 #endif
 }
 
-// traversal index (over the OWNED sites of one parity) -> site; all indices stay in registers
-__device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int parity, SiteNbr& s) {
+// traversal index (over the OWNED sites of one parity) -> (x/2, y, z, interior t); all indices stay in registers
+__device__ __forceinline__ void traversal_coords(const Geom& g, unsigned tix, unsigned& xh, unsigned& y, unsigned& z, unsigned& ti) {
     const unsigned row = (unsigned)g.Lxh, pl = row * (unsigned)g.L[1];
+    if (g.Bz * g.Bt > 1) {
+        // block tiles: (z-chunk, t-block, z-block, x-y segment group | warp: segment, t in block, z in block | lane)
+        const unsigned wb = (unsigned)g.Wb, bz = (unsigned)g.Bz, bt = (unsigned)g.Bt, sw = wb / (bz * bt);
+        const unsigned W = tix >> 5, lane = tix & 31u, blk = W / wb, w = W - blk * wb;
+        const unsigned dz = w % bz, dt = (w / bz) % bt, sl = w / (bz * bt);
+        const unsigned sgroups = (pl >> 5) / sw, nzb = (unsigned)g.Zc / bz, ntb = (unsigned)g.Lt_int / bt;
+        unsigned q = blk;
+        const unsigned sb = q % sgroups; q /= sgroups;
+        const unsigned zb = q % nzb;     q /= nzb;
+        const unsigned tb = q % ntb;
+        const unsigned zc = q / ntb;
+        const unsigned r = ((sb * sw + sl) << 5) + lane;
+        y = r / row; xh = r - y * row;
+        z = zc * (unsigned)g.Zc + zb * bz + dz;
+        ti = tb * bt + dt;
+        return;
+    }
     const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
     const unsigned zc = tix / span;  unsigned r = tix - zc * span;
-    const unsigned ti = r / grp;     r -= ti * grp;
+    ti = r / grp;                    r -= ti * grp;
     const unsigned zi = r / pl;      r -= zi * pl;
-    const unsigned y = r / row;
-    const unsigned xh = r - y * row;
-    const unsigned z = zc * (unsigned)g.Zc + zi;
-    const unsigned t = ti + (unsigned)g.t_halo;                          // stored time slice
-    site_from_coords(g, xh, y, z, t, parity, s);
+    y = r / row;
+    xh = r - y * row;
+    z = zc * (unsigned)g.Zc + zi;
+}
+__device__ __forceinline__ void site_of_thread(const Geom& g, unsigned tix, int parity, SiteNbr& s) {
+    unsigned xh, y, z, ti;
+    traversal_coords(g, tix, xh, y, z, ti);
+    site_from_coords(g, xh, y, z, ti + (unsigned)g.t_halo, parity, s);          // stored time slice
 }
 
 // slab mode: 1 = the thread's site lies in the first owned time slice, 2 = in the last one, 0 otherwise.
 // Recomputed from the traversal index at store time so that nothing stays live across the kernel body.
 __device__ __forceinline__ int slab_edge(const Geom& g, unsigned tix) {
     if (!g.t_halo) return 0;
-    const unsigned grp = (unsigned)g.Lxh * (unsigned)g.L[1] * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
-    const unsigned ti = (tix % span) / grp;
+    unsigned xh, y, z, ti;
+    traversal_coords(g, tix, xh, y, z, ti);
     return (ti == 0 ? 1 : 0) | ((int)ti + 1 == g.Lt_int ? 2 : 0);
+}
+
+// L2 prefetch ahead of the traversal (su_set_option "prefetch_slices"). The traversal walks up in t inside a z-chunk,
+// and the links of the slice above are the only ones a sub-step touches for the first time (DESIGN.md "Traversal
+// order"); with few warps per SM (fused launches) nothing hides their DRAM latency. So every warp, before it starts on
+// its 32 sites, asks L2 for the eight link tiles (4 mu x 2 parities, E * 512 B each, contiguous in the tiled layout)
+// that hold the same sites k time slices further up: one cp.async.bulk.prefetch.L2 per (mu, parity), issued by lanes
+// 0..7. A hint only: it moves no data into the SM, orders nothing and cannot change a result.
+__device__ __forceinline__ void l2_prefetch_bulk(const void* p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+template <int E, class T2>
+__device__ __forceinline__ void prefetch_slices_ahead(const void* links, const Geom& g, unsigned cb0, int k) {
+    constexpr unsigned BYTES = E * LINK_TILE * sizeof(T2);
+    if (BYTES % 16 != 0) return;
+    const unsigned lane = threadIdx.x & 31u;
+    if (lane < 8) {
+        const unsigned cbT = (unsigned)(((unsigned long long)cb0 + (unsigned long long)k * g.Vsh) % g.Vh);
+        const T2* p = (const T2*)links + (size_t)lane * E * g.Vhp + (size_t)(cbT / LINK_TILE) * (E * LINK_TILE);
+        l2_prefetch_bulk(p, BYTES);
+    }
 }
 
 // FUSE3: each staple term S += A B C (three links) is evaluated row by row with all three operands
@@ -138,7 +181,7 @@ __device__ __forceinline__ int slab_edge(const Geom& g, unsigned tix) {
 // LDN: how neighbour links are loaded (LD_RO in a plain launch, LD_COHERENT in a fused one).
 //
 // update_link: staple, W = U S^dagger, subgroup loop and store for ONE link U_mu(x), x = s (rows a1-a6).
-template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, bool FUSE3, bool KUNR, int LDN, int PRE, bool FUSED>
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int FUSE3, bool KUNR, int LDN, int PRE, bool FUSED>
 __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, const int mu, const SiteNbr& s, const unsigned tix,
                                             const unsigned warp_mask, const uint32_t sweep_ctr, T* dir_col,
                                             unsigned& att_total, unsigned& exhausted) {
@@ -151,7 +194,22 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
     const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
     // heatbath, register kernels: the directions of all subgroup draws are link-independent; evaluate them
     // now, in the shadow of the first loads, and park them in shared memory (one private column per thread)
-    if (PRE >= 1) {
+    // PRE == 4: the same quantities, but draw q is evaluated in the shadow of the loads of staple term 6 q / NSUB
+    // (between issuing a term's three links and multiplying them), where the warp would otherwise only wait
+    auto pre_draw = [&](int q) {
+        T n[3], Q, R;
+        kp_direction<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2((int)a.pass, p, mu, q), n);
+        kp_attempt0<T>(a.k0, a.k1, s.lex, sweep_ctr, pack_c2((int)a.pass, p, mu, q), Q, R);
+        dir_col[(3 * q) * BLOCK] = n[0]; dir_col[(3 * q + 1) * BLOCK] = n[1]; dir_col[(3 * q + 2) * BLOCK] = n[2];
+        dir_col[(3 * NSUB + 2 * q) * BLOCK] = Q; dir_col[(3 * NSUB + 2 * q + 1) * BLOCK] = R;
+    };
+    auto pre_slot = [&](int slot) {
+        if (PRE == 4) {
+#pragma unroll
+            for (int q = 0; q < NSUB; ++q) if ((q * 6) / NSUB == slot) pre_draw(q);
+        }
+    };
+    if (PRE >= 1 && PRE != 4) {
 #pragma unroll
         for (int q = 0; q < NSUB; ++q) {
             T n[3];
@@ -159,7 +217,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
             dir_col[(3 * q) * BLOCK] = n[0]; dir_col[(3 * q + 1) * BLOCK] = n[1]; dir_col[(3 * q + 2) * BLOCK] = n[2];
         }
     }
-    if (PRE >= 2) {
+    if (PRE >= 2 && PRE != 4) {
 #pragma unroll
         for (int q = 0; q < NSUB; ++q) {
             T Q, R;
@@ -171,6 +229,74 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
     C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
     M::zero(S);
     const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
+    typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
+    constexpr bool STREAM_SELF = !FUSED || SUG_FUSED_STREAM;
+    if (FUSE3 == 3) {
+        // two-row storage with lazy third rows (Su3Rows): three links up front per term, as FUSE3 == 1
+        static_assert(FUSE3 != 3 || (STORE == STORE_RECON12 && NC == 3 && UNR), "FUSE3 == 3 is the SU(3) two-row form");
+#pragma unroll(KUNR ? 3 : 1)
+        for (int k = 0; k < 3; ++k) {
+            const int nu = k + (k >= mu ? 1 : 0);
+            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+            const typename IO::T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
+            const typename IO::T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
+            IO::template load_stored<LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
+            IO::template load_stored<LDN>(pl_nu_o, cb + (unsigned)dpmu, P);
+            IO::template load_stored<LDN>(pl_nu_s, cb, A);
+            pre_slot(2 * k);
+            Su3Rows<T>::acc_upper(S, A, B, P);
+            if (LDT != LDN && nu == 3) {
+                IO::template load_stored<LDT>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load_stored<LDT>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load_stored<LDT>(pl_nu_o, cb + (unsigned)dmnu, A);
+            } else {
+                IO::template load_stored<LDN>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load_stored<LDN>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load_stored<LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
+            }
+            pre_slot(2 * k + 1);
+            Su3Rows<T>::acc_lower(S, A, B, P);
+        }
+    } else if (FUSE3 == 2) {
+        // Software pipeline over the six staple terms (few warps per SM: nothing else hides the load latency). A term is
+        // P = A B (or A^dagger B), then S += P C^dagger (or P C). While P is formed the term's third link C is in
+        // flight; while S is accumulated the first two links of the NEXT term are (the own link after the last
+        // term). Same sums in the same order as mul_nn + acc_nd / mul_dn + acc_nn, i.e. as the FUSE3 == 1 form.
+        C Cm[NC * NC];
+        auto nu_of = [&](int k) { return k + (k >= mu ? 1 : 0); };
+        auto load_ab = [&](int t) {       // first two links of term t (t = 2 k: upper, 2 k + 1: lower)
+            const int nu = nu_of(t >> 1);
+            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]), dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+            if (!(t & 1)) {               // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
+                IO::template load<LDN>(IO::plane((const void*)a.links, a.g, nu, p), cb, A);
+                IO::template load<LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
+            } else if (LDT != LDN && nu == 3) {   // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu); slice below: evict-first
+                IO::template load<LDT>(IO::plane((const void*)a.links, a.g, nu, 1 - p), cb + (unsigned)dmnu, A);
+                IO::template load<LDT>(pl_mu_o, cb + (unsigned)dmnu, B);
+            } else {
+                IO::template load<LDN>(IO::plane((const void*)a.links, a.g, nu, 1 - p), cb + (unsigned)dmnu, A);
+                IO::template load<LDN>(pl_mu_o, cb + (unsigned)dmnu, B);
+            }
+        };
+        auto load_c = [&](int t) {
+            const int nu = nu_of(t >> 1);
+            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+            if (!(t & 1))                        IO::template load<LDN>(IO::plane((const void*)a.links, a.g, nu, 1 - p), cb + (unsigned)dpmu, Cm);
+            else if (LDT != LDN && nu == 3)      IO::template load<LDT>(IO::plane((const void*)a.links, a.g, nu, p), cb + (unsigned)(dmnu + dpmu), Cm);
+            else                                 IO::template load<LDN>(IO::plane((const void*)a.links, a.g, nu, p), cb + (unsigned)(dmnu + dpmu), Cm);
+        };
+        load_ab(0);
+#pragma unroll
+        for (int t = 0; t < 6; ++t) {
+            load_c(t);
+            if (!(t & 1)) M::mul_nn(A, B, P); else M::mul_dn(A, B, P);
+            if (t < 5) load_ab(t + 1);
+            else IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, A);       // the own link U
+            pre_slot(t);
+            if (!(t & 1)) M::acc_nd(S, P, Cm); else M::acc_nn(S, P, Cm);
+        }
+    } else {
 #pragma unroll(KUNR ? 3 : 1)
     for (int k = 0; k < 3; ++k) {
         const int nu = k + (k >= mu ? 1 : 0);
@@ -183,6 +309,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
             IO::template load<LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
             IO::template load<LDN>(pl_nu_o, cb + (unsigned)dpmu, P);
             IO::template load<LDN>(pl_nu_s, cb, A);
+            pre_slot(2 * k);
             M::acc_nnd(S, A, B, P);
             // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
             if (LDT != LDN && k == 2 && nu == 3) {
@@ -196,6 +323,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
                 IO::template load<LDN>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
                 IO::template load<LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
             }
+            pre_slot(2 * k + 1);
             M::acc_dnn(S, A, B, P);
         } else {
             // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
@@ -212,11 +340,10 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
             M::acc_nn(S, P, A);
         }
     }
-    typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
+    }
     C* U = A;
     C* W = B;
-    constexpr bool STREAM_SELF = !FUSED || SUG_FUSED_STREAM;
-    IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, U);
+    if (FUSE3 != 2) IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, U);
     M::mul_nd(U, S, W);                                   // W = U S^dagger
     update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex, sweep_ctr,
                                        pack_c2((int)a.pass, p, mu, 0),
@@ -273,10 +400,11 @@ __device__ __forceinline__ void fused_wait(const UpdateArgs::Fused& fz, int s, i
     __syncwarp();
 }
 
-template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, bool FUSE3 = false, bool KUNR = false, bool FUSED = false>
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, int FUSE3 = 0, bool KUNR = false, bool FUSED = false>
 __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
     constexpr int NSUB = NC * (NC - 1) / 2;
-    constexpr int PRE = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
+    constexpr int PRE_ASKED = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
+    constexpr int PRE = (PRE_ASKED == 4 && !FUSE3) ? (sizeof(T) == 4 ? 1 : 0) : PRE_ASKED;     // 4 needs the three-link staple terms
     __shared__ T dir_sm[PRE >= 2 ? 5 * NSUB : (PRE == 1 ? 3 * NSUB : 1)][PRE ? BLOCK : 1];
     const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
     unsigned att_total = 0, exhausted = 0;
@@ -287,6 +415,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
         if (active) {
             SiteNbr s;
             site_of_thread(a.g, tix, a.parity, s);
+            if (a.pf_slices > 0)
+                prefetch_slices_ahead<LinkIO<NC, T, STORE, UNR>::E, typename V2<T>::type>(a.links, a.g, __shfl_sync(warp_mask, s.cb, 0), a.pf_slices);
             update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, LD_RO, PRE, false>(
                 a, a.parity, a.mu, s, tix, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
         }
@@ -327,6 +457,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
                 const int p = fused_parity(a.fz.fg, st), mu = fused_mu(a.fz.fg, st);
                 SiteNbr s;
                 site_from_coords(a.g, xh, y, zu * (unsigned)a.fz.fg.U + zi, t, p, s);
+                if (a.pf_slices > 0 && st == 0)             // the first stage is the one that touches links for the first time
+                    prefetch_slices_ahead<LinkIO<NC, T, STORE, UNR>::E, typename V2<T>::type>(a.links, a.g, __shfl_sync(warp_mask, s.cb, 0), a.pf_slices);
                 update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, SUG_FUSED_LD, PRE, true>(
                     a, p, mu, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
             }

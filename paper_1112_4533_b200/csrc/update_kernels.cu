@@ -1,6 +1,9 @@
 // update_kernels.cu — instantiation and launch of the staple + link-update kernel
 // (update_kernel.cuh) for one (parity, mu) sub-step. Compiled once per colour count with
 // -DSUG_NC=<Nc>. Block size / minimum blocks per SM per variant: DESIGN.md "Launch configuration".
+#include <map>
+#include <mutex>
+
 #include "su_internal.h"
 #include "update_rows_kernel.cuh"
 
@@ -15,10 +18,25 @@ namespace sug {
 
 // One launch configuration: threads per block, the __launch_bounds__ minimum blocks per SM (= the
 // register cap), and the kernel-structure switches of k_update (FUSE3, KUNR).
-template <int BLOCK_, int MINB_, bool FUSE3_ = false, bool KUNR_ = false> struct Cfg {
-    static constexpr int BLOCK = BLOCK_, MINB = MINB_;
-    static constexpr bool FUSE3 = FUSE3_, KUNR = KUNR_;
+template <int BLOCK_, int MINB_, int FUSE3_ = 0, bool KUNR_ = false> struct Cfg {
+    static constexpr int BLOCK = BLOCK_, MINB = MINB_, FUSE3 = FUSE3_;       // FUSE3: 0 two-step, 1 three links up front, 2 software-pipelined
+    static constexpr bool KUNR = KUNR_;
 };
+
+// a.dyn_smem (su_set_option "blocks_per_sm"): unused dynamic shared memory requested with the launch, which caps the
+// resident blocks per SM below what the registers allow - fused launches re-use links through L2 only while the
+// blocks in flight cover less lattice than L2 holds.
+template <class K> static void launch_k(K kern, unsigned grid, int block, cudaStream_t st, const UpdateArgs& a) {
+    if (a.dyn_smem > 48 * 1024) {                 // above the default limit a kernel has to be opted in once
+        static std::mutex mu;
+        static std::map<const void*, int> granted;
+        std::lock_guard<std::mutex> lock(mu);
+        int& have = granted[(const void*)kern];
+        if (a.dyn_smem > have && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, a.dyn_smem) == cudaSuccess)
+            have = a.dyn_smem;
+    }
+    kern<<<grid, block, a.dyn_smem, st>>>(a);
+}
 
 // a.fz.work != NULL: the fused launch of a.fz.fg.g consecutive sub-steps (fused_schedule.h), one block per ticket
 template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB>
@@ -26,12 +44,12 @@ static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t s
     const bool fused = a.fz.work != nullptr;
     if (kind == KIND_HB) {
         const unsigned grid = (a.g.Vh_int + HB::BLOCK - 1) / HB::BLOCK;
-        if (fused) k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR, true><<<a.fz.n_tickets, HB::BLOCK, 0, st>>>(a);
-        else       k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR><<<grid, HB::BLOCK, 0, st>>>(a);
+        if (fused) launch_k(k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR, true>, a.fz.n_tickets, HB::BLOCK, st, a);
+        else       launch_k(k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR>, grid, HB::BLOCK, st, a);
     } else {
         const unsigned grid = (a.g.Vh_int + OR::BLOCK - 1) / OR::BLOCK;
-        if (fused) k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR, true><<<a.fz.n_tickets, OR::BLOCK, 0, st>>>(a);
-        else       k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR><<<grid, OR::BLOCK, 0, st>>>(a);
+        if (fused) launch_k(k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR, true>, a.fz.n_tickets, OR::BLOCK, st, a);
+        else       launch_k(k_update<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR>, grid, OR::BLOCK, st, a);
     }
     return cudaGetLastError();
 }
@@ -45,11 +63,17 @@ template <class HB, class OR = HB> static int spb_t(int kind) { return kind == K
 #ifndef SUG_SU3_F64_MINB
 #define SUG_SU3_F64_MINB 3
 #endif
+#ifndef SUG_SU3_F64_SMODE
+#define SUG_SU3_F64_SMODE 1
+#endif
+#ifndef SUG_SU3_F64_HB_MINB
+#define SUG_SU3_F64_HB_MINB SUG_SU3_F64_MINB
+#endif
 #ifndef SUG_CFG_SU3_F64_HB
-#define SUG_CFG_SU3_F64_HB Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, true, true>
+#define SUG_CFG_SU3_F64_HB Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_HB_MINB, SUG_SU3_F64_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3_F64_OR
-#define SUG_CFG_SU3_F64_OR Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, true, true>
+#define SUG_CFG_SU3_F64_OR Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, SUG_SU3_F64_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3_F32_HB
 #define SUG_CFG_SU3_F32_HB Cfg<128, 4, true, true>
@@ -57,17 +81,30 @@ template <class HB, class OR = HB> static int spb_t(int kind) { return kind == K
 #ifndef SUG_CFG_SU3_F32_OR
 #define SUG_CFG_SU3_F32_OR Cfg<128, 5, true, true>
 #endif
+// two-row storage: staple form (1: every link completed on load, 3: lazy third rows, Su3Rows) and register caps
+#ifndef SUG_SU3R_SMODE
+#define SUG_SU3R_SMODE 3
+#endif
+#ifndef SUG_SU3R_F64_MINB
+#define SUG_SU3R_F64_MINB 3
+#endif
+#ifndef SUG_SU3R_F32_MINB
+#define SUG_SU3R_F32_MINB 3
+#endif
+#ifndef SUG_SU3R_F32_HB_MINB
+#define SUG_SU3R_F32_HB_MINB SUG_SU3R_F32_MINB
+#endif
 #ifndef SUG_CFG_SU3R_F64_HB
-#define SUG_CFG_SU3R_F64_HB Cfg<128, 3, true, true>
+#define SUG_CFG_SU3R_F64_HB Cfg<128, SUG_SU3R_F64_MINB, SUG_SU3R_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3R_F64_OR
-#define SUG_CFG_SU3R_F64_OR Cfg<128, 3, true, true>
+#define SUG_CFG_SU3R_F64_OR Cfg<128, SUG_SU3R_F64_MINB, SUG_SU3R_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3R_F32_HB
-#define SUG_CFG_SU3R_F32_HB Cfg<128, 1>
+#define SUG_CFG_SU3R_F32_HB Cfg<128, SUG_SU3R_F32_HB_MINB, SUG_SU3R_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3R_F32_OR
-#define SUG_CFG_SU3R_F32_OR Cfg<128, 3, true, true>
+#define SUG_CFG_SU3R_F32_OR Cfg<128, SUG_SU3R_F32_MINB, SUG_SU3R_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU4_F64_HB
 #define SUG_CFG_SU4_F64_HB Cfg<128, 1>
