@@ -86,6 +86,20 @@ def ncu_traffic(tag):
     return None
 
 
+def ncu_l2_bytes(tag):
+    """L2 -> SM bytes per launch of the dominant kernel (ncu l1tex__m_xbar2l1tex_read_bytes.sum, committed), or None."""
+    p = os.path.join(ROOT, "profiles", "l2_traffic.csv")
+    try:
+        with open(p) as f:
+            for line in f.read().splitlines()[1:]:
+                t, b = line.split(",")[:2]
+                if t == tag:
+                    return float(b)
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -569,6 +583,7 @@ def run_slabs(args, wl, torch, dist, rank, world, local, warmup, recon12):
 
 
 FMA_PEAKS = {}        # precision -> measured TFLOP/s of the FMA pipe (su_measure_fma_peak), filled once per run
+L2_PEAK = {}          # {"gbs", "bytes_per_clk"} of the L2 -> SM read path (su_measure_l2_peak), filled once per run
 
 
 def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
@@ -609,6 +624,24 @@ def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
                 "update_kernels_share_of_step": ((or_ms * N_OR * 8 + (hb_ms or 0.0) * N_HB * 8) / (res["ms"] / steps)),
                 "traffic": ncu_traffic(f"su{Nc}_{precision}_{'recon12' if recon12 else 'full'}_or"),
                 "traffic_source": "profiles/traffic.csv (ncu --set full of this kernel, committed; not re-measured in this run)"}
+        # Third figure: the L2 -> SM read path. A link update issues 19 link loads (18 staple links + the own link) and L1
+        # serves < 10 % of them, so ~19 R s bytes per update cross the L2 fabric, 2.1 x the 9 R s that must cross HBM. The
+        # path delivers 11 kB per SM clock chip-wide (su_measure_l2_peak, = 94 % of the 11.8 kB / clock ncu states), and the
+        # kernel uses 0.5 - 0.6 of that: reported so that the reader can rule this roof out (profiles/r02g).
+        loaded = 19 * reals_per_link(Nc, recon12) * (8 if precision == "fp64" else 4) * (V // 2)
+        xbar = ncu_l2_bytes(f"su{Nc}_{precision}_{'recon12' if recon12 else 'full'}_or")
+        if L2_PEAK.get("gbs"):
+            l2_bytes = xbar if xbar else loaded
+            l2_ach = l2_bytes / (or_ms * 1e-3) / 1e9
+            sm_mhz = (res.get("clocks") or {}).get("sm_mhz")
+            run_peak = L2_PEAK["bytes_per_clk"] * sm_mhz * 1e6 / 1e9 if sm_mhz and L2_PEAK.get("bytes_per_clk") else None
+            roof["l2"] = {"achieved_gbs": l2_ach, "peak_gbs_burst_clock": L2_PEAK["gbs"], "frac_of_burst_peak": l2_ach / L2_PEAK["gbs"],
+                          "peak_bytes_per_sm_clock": L2_PEAK.get("bytes_per_clk"), "sm_mhz_in_run": sm_mhz,
+                          "peak_gbs_at_run_clock": run_peak, "frac_at_run_clock": (l2_ach / run_peak) if run_peak else None,
+                          "bytes_per_launch": l2_bytes, "link_loads_issued_bytes_per_launch": loaded,
+                          "bytes_source": ("profiles/l2_traffic.csv (ncu l1tex__m_xbar2l1tex_read_bytes.sum of this kernel, committed)"
+                                           if xbar else "19 link loads per update, no L1 hits assumed"),
+                          "peak_source": "measured in this run (su_measure_l2_peak: 24 MB L2-resident buffer, ld.global.cg)"}
     return {"value": value, "ms_per_step": res["ms"] / steps, "gflops": n_ranks * flops_step / t_step / 1e9,
             "effective_gbs": n_ranks * bpu * updates_step / t_step / 1e9, "roofline": roof}
 
@@ -672,6 +705,8 @@ def main():
         args.parallel = "slabs" if world > 1 else "replicas"
     for prec in {args.precision, "fp32", "fp64"}:
         FMA_PEAKS[prec] = su.measure_fma_peak(prec, local)[0]
+    g, _, bpc = su.measure_l2_peak(local)
+    L2_PEAK.update({"gbs": g, "bytes_per_clk": bpc})
     if args.config_table:
         return run_config_table(args, torch, su, local, peak)
     if args.parallel == "slabs":
@@ -738,7 +773,7 @@ def main():
                            "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)"},
                 "gflops": main_num["gflops"], "effective_hbm_gbs": main_num["effective_gbs"],
                 "flop_formula": "13*mm+10Nc^2 + n_sub*(23+56Nc) [OR] / n_sub*(57+13*1.05+56Nc) [HB], mm=8Nc^3-2Nc^2 (DESIGN.md)",
-                "fma_peaks_tflops": dict(FMA_PEAKS),
+                "fma_peaks_tflops": dict(FMA_PEAKS), "l2_peak": dict(L2_PEAK),
                 "roofline": main_num["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": res["launches"],
                 "clocks": res["clocks"], "plaquette": res["plaquette"], "polyakov": res["polyakov"],
                 "kp_exhausted": res["kp_exhausted"], "variants": variants}

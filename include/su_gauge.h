@@ -189,6 +189,18 @@ su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* o
  *                     su_reunitarize); the other kernels run the reunitarisation kernel at the end of the sweep. This
  *                     one DOES change results at rounding level against su_sweep + su_reunitarize (later sub-steps of
  *                     the last pass already see projected neighbours); su_sweep without it never reunitarises. 0: off.
+ *   "coop_sweep"      1: su_sweep runs all heatbath passes of a sweep in ONE cooperative launch and all overrelaxation
+ *                     passes in another, with grid barriers where the launch boundaries were (register kernels of
+ *                     Nc <= 4, lattices whose V/2 threads are resident at once, not slabs; otherwise plain launches;
+ *                     su_get_option "coop_sweep_effective": bit 0 heatbath, bit 1 overrelaxation). Bitwise the plain
+ *                     sweep (tested). Measured no faster than the CUDA-graph replay of the 40 launches (profiles/r02g).
+ *   "block_tile_z", "block_tile_t"   the warps of a thread block of the Nc = 3, 4 register kernels work on the same x-y
+ *                     segments of this many consecutive z-planes / time slices (1: a block is consecutive segments of
+ *                     one plane), dropped silently where the lattice or the block does not divide evenly.
+ *   "prefetch_slices" k > 0: every warp of an update kernel asks L2 (cp.async.bulk.prefetch.L2) for the link tiles of
+ *                     its sites' positions k time slices ahead of the traversal. A hint; 0 (default) = off.
+ *   "blocks_per_sm"   n > 0: update launches request unused dynamic shared memory so that only n blocks fit an SM.
+ *                     (measurement knob: it also shrinks L1, which the loads in flight need; profiles/r02g.)
  * Unknown names: SU_EINVAL. */
 su_status su_set_option(su_lattice*, const char* name, long long value);
 su_status su_get_option(su_lattice*, const char* name, long long* value);
@@ -211,12 +223,14 @@ int su_fused_dep_debug(int Lx, int Ly, int Lz, int Lt, int sites_per_block, int 
 su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double* ms);
 
 /* Measured L2 -> SM read throughput of the device in GB/s: every thread block streams one 24 MB L2-resident buffer
- * with 128-bit loads that bypass L1 (4 blocks of 256 threads per SM, 8 loads per thread in flight, best of 5
- * launches). The staple + update kernel issues 19 link loads per update of which L1 serves < 10 %, so this, not
- * HBM, is the roof it runs on for 18-real SU(3) (profiles/r02g). device -1 = current.
+ * with 128-bit loads that bypass L1 (through_l1 = 0: ld.global.cg) or allocate in it (through_l1 = 1: ld.global.nc, each
+ * block's 24 MB still far beyond L1) (4 blocks of 256 threads per SM, 8 loads per thread in flight, best of 5
+ * launches). The staple + update kernel issues 19 link loads per update of which L1 serves < 10 %, so 2.1 x its HBM
+ * bytes cross this path; bench.py reports the fraction of this rate it uses (0.5 - 0.6 for 18-real SU(3): not the
+ * limiter, profiles/r02g). device -1 = current.
  * ms (may be NULL): duration of the best launch; bytes_per_clock (may be NULL): the same throughput per SM clock
  * cycle (clock64 span of one block), the figure that carries over to a run at another clock. Synchronises the device. */
-su_status su_measure_l2_peak(int device, double* gbs, double* ms, double* bytes_per_clock);
+su_status su_measure_l2_peak(int device, int through_l1, double* gbs, double* ms, double* bytes_per_clock);
 
 /* Text of the last error on this handle ("" if none); static text if the handle is NULL.
  * Owned by the library, valid until the next call on the handle. */

@@ -98,7 +98,7 @@ def lib():
     L.su_save_config.argtypes = [P, C.c_char_p]
     L.su_load_config.argtypes = [P, C.c_char_p]
     L.su_measure_fma_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D)]
-    L.su_measure_l2_peak.argtypes = [I, C.POINTER(D), C.POINTER(D), C.POINTER(D)]
+    L.su_measure_l2_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D), C.POINTER(D)]
     L.su_set_option.argtypes = [P, C.c_char_p, C.c_longlong]
     L.su_get_option.argtypes = [P, C.c_char_p, C.POINTER(C.c_longlong)]
     for name in ABI_SYMBOLS:
@@ -129,10 +129,10 @@ def measure_fma_peak(precision="fp64", device=-1):
     return t.value, ms.value
 
 
-def measure_l2_peak(device=-1):
+def measure_l2_peak(device=-1, through_l1=False):
     """-> (GB/s, ms of the best launch, bytes per SM clock) of the device's L2 -> SM read path (su_measure_l2_peak)"""
     g, ms, bpc = C.c_double(), C.c_double(), C.c_double()
-    st = lib().su_measure_l2_peak(device, C.byref(g), C.byref(ms), C.byref(bpc))
+    st = lib().su_measure_l2_peak(device, 1 if through_l1 else 0, C.byref(g), C.byref(ms), C.byref(bpc))
     if st != SU_OK:
         raise SuError(st, "su_measure_l2_peak")
     return g.value, ms.value, bpc.value

@@ -49,6 +49,8 @@ struct su_lattice {
     int prefetch_slices = 0;         // update kernels: L2 prefetch distance in time slices (0: off)
     int blocks_per_sm = 0;           // update kernels: cap on the resident blocks per SM (0: whatever fits)
     int tile_z = 1, tile_t = 1;      // register update kernels: z-planes x time slices per block tile (Geom::Bz, Bt)
+    bool coop_sweep = false;         // su_sweep: one cooperative launch per kind (all its passes) when the lattice fits the device at once
+    long long coop_sites[2] = {-1, -1};   // cached capacity (sites of one parity) of the cooperative kernel per kind; -1: not queried
     bool reunit_on_store = false;    // su_sweep leaves reunitarised links (in its last pass; see su_set_option)                     // slab mode: false between su_import_links and su_slab_halo_push
     uint64_t seed = 0;
     uint32_t sweep = 0;
@@ -176,6 +178,7 @@ __global__ void __launch_bounds__(256) k_fma_peak(T* out, const T* in, int iters
 
 // L2 -> SM throughput micro-benchmark (su_measure_l2_peak): every block streams the whole L2-resident buffer with
 // 128-bit loads that bypass L1 (ld.global.cg), 8 independent loads per thread in flight; the sum keeps them alive.
+template <int MODE>      // 0: ld.global.cg (L2 only), 1: ld.global.nc (through L1, as the update kernels' neighbour loads)
 __global__ void __launch_bounds__(256) k_l2_peak(double* out, const double2* __restrict__ buf, size_t n16, int passes) {
     double acc = 0;
     const long long c0 = clock64();
@@ -186,7 +189,7 @@ __global__ void __launch_bounds__(256) k_l2_peak(double* out, const double2* __r
         for (size_t done = 0; done < n16; done += stride) {
             double2 v[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) { size_t j = i + (size_t)k * blockDim.x; if (j >= n16) j -= n16; v[k] = __ldcg(buf + j); }
+            for (int k = 0; k < 8; ++k) { size_t j = i + (size_t)k * blockDim.x; if (j >= n16) j -= n16; v[k] = MODE == 0 ? __ldcg(buf + j) : __ldg(buf + j); }
 #pragma unroll
             for (int k = 0; k < 8; ++k) acc += v[k].x + v[k].y;
             i += stride; if (i >= n16) i -= n16;
@@ -214,6 +217,21 @@ int update_spb(su_lattice* h, int kind) {
         case 8: return update_spb_nc8(h->var, kind);
         default: return 0;
     }
+}
+
+// "coop_sweep": the whole-pass cooperative kernel can be used when it exists for this variant, the handle is not a slab
+// and every block of a sub-step is resident at once
+bool coop_fits(su_lattice* h, int kind) {
+    if (!h->coop_sweep || h->g.t_halo) return false;
+    if (h->coop_sites[kind] < 0) {
+        switch (h->Nc) {
+            case 2: h->coop_sites[kind] = update_coop_sites_nc2(h->var, kind); break;
+            case 3: h->coop_sites[kind] = update_coop_sites_nc3(h->var, kind); break;
+            case 4: h->coop_sites[kind] = update_coop_sites_nc4(h->var, kind); break;
+            default: h->coop_sites[kind] = 0;
+        }
+    }
+    return (long long)h->g.Vh_int <= h->coop_sites[kind];
 }
 
 // fused launches need the whole lattice in one buffer with periodic t (no slab halos) and a kernel that has the fused form
@@ -355,6 +373,20 @@ su_status enqueue_sweep(su_lattice* h, double beta, int n_hb, int n_or, const ui
         const int kind = pass < n_hb ? KIND_HB : KIND_OR;
         const bool ru = reunit_store && pass == n_hb + n_or - 1;
         if (timed && pass == n_hb) SU_CUDA(h, cudaEventRecord(ev.e[1], h->stream), "timing event");
+        if (coop_fits(h, kind)) {
+            // all the passes of this kind in ONE cooperative launch (grid barriers between the sub-steps)
+            const int n_kind = kind == KIND_HB ? n_hb : n_or, last = n_hb + n_or - 1;
+            UpdateArgs a{};
+            a.links = h->links; a.g = h->g; a.parity = 0; a.mu = 0; a.beta = beta;
+            a.k0 = (uint32_t)h->seed; a.k1 = (uint32_t)(h->seed >> 32);
+            a.sweep = h->sweep; a.sweep_ptr = d_sweep; a.pass = kind == KIND_HB ? (uint32_t)pass : 0u;
+            a.attempts = nullptr; a.counters = h->d_counters;
+            a.reunit = (reunit_store && pass + n_kind - 1 == last) ? 1 : 0;
+            a.coop_passes = n_kind;
+            SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "cooperative update kernel launch");
+            pass += n_kind - 1;
+            continue;
+        }
         const int g = effective_fuse(h, kind);
         if (g > 1) {
             for (int sub0 = 0; sub0 < 8; sub0 += g) {        // sub-step index = 4 parity + mu (reading R6)
@@ -950,6 +982,13 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
         h->reunit_on_store = value != 0;
         return SU_OK;
     }
+    if (!strcmp(name, "coop_sweep")) {
+        if (value != 0 && value != 1) return fail(h, SU_EINVAL, "coop_sweep must be 0 or 1");
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);
+        h->coop_sweep = value != 0;
+        return SU_OK;
+    }
     if (!strcmp(name, "block_tile_z") || !strcmp(name, "block_tile_t")) {
         if (value < 1 || value > 8) return fail(h, SU_EINVAL, "%s must be in 1...8", name);
         SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
@@ -987,6 +1026,8 @@ su_status su_get_option(su_lattice* h, const char* name, long long* value) {
     if (!h || !name || !value) return SU_EINVAL;
     if (!strcmp(name, "z_chunk_planes")) { *value = h->g.Zc; return SU_OK; }
     if (!strcmp(name, "reunit_on_store")) { *value = h->reunit_on_store ? 1 : 0; return SU_OK; }
+    if (!strcmp(name, "coop_sweep")) { *value = h->coop_sweep ? 1 : 0; return SU_OK; }
+    if (!strcmp(name, "coop_sweep_effective")) { *value = (coop_fits(h, 0) ? 1 : 0) | (coop_fits(h, 1) ? 2 : 0); return SU_OK; }
     if (!strcmp(name, "block_tile_z")) { *value = h->tile_z; return SU_OK; }
     if (!strcmp(name, "block_tile_t")) { *value = h->tile_t; return SU_OK; }
     if (!strcmp(name, "prefetch_slices")) { *value = h->prefetch_slices; return SU_OK; }
@@ -1052,7 +1093,7 @@ su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double
     return SU_OK;
 }
 
-su_status su_measure_l2_peak(int device, double* gbs, double* ms, double* bytes_per_clock) {
+su_status su_measure_l2_peak(int device, int through_l1, double* gbs, double* ms, double* bytes_per_clock) {
     if (!gbs) return SU_EINVAL;
     int dev = device;
     if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return SU_ECUDA;
@@ -1072,7 +1113,8 @@ su_status su_measure_l2_peak(int device, double* gbs, double* ms, double* bytes_
         cudaMemset(buf, 0, bytes);
         for (int rep = 0; rep < 6 && st == SU_OK; ++rep) {          // first repetition = warm-up (brings the buffer into L2)
             cudaEventRecord(e0, 0);
-            k_l2_peak<<<blocks, threads>>>((double*)out, (const double2*)buf, n16, passes);
+            if (through_l1) k_l2_peak<1><<<blocks, threads>>>((double*)out, (const double2*)buf, n16, passes);
+            else            k_l2_peak<0><<<blocks, threads>>>((double*)out, (const double2*)buf, n16, passes);
             cudaEventRecord(e1, 0);
             if (cudaEventSynchronize(e1) != cudaSuccess) { st = SU_ECUDA; break; }
             float t = 0;

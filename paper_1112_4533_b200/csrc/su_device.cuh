@@ -135,7 +135,18 @@ template <class T> __device__ __forceinline__ void su3_third_row(cx<T>* m) {   /
 // link being updated: touched once per sub-step, so it should not displace re-used lines).
 // LD_COHERENT = ld.relaxed.gpu (served by L2, never by a stale L1 line): links that another block may have
 // rewritten earlier in the SAME launch (fused multi-sub-step launches, fused_schedule.h).
-enum : int { LD_PLAIN = 0, LD_RO = 1, LD_STREAM = 2, LD_COHERENT = 3 };
+// LD_CG = ld.global.cg (cached in L2 only), LD_NA = ld.global.nc.L1::no_allocate (read-only path, no L1 line kept).
+enum : int { LD_PLAIN = 0, LD_RO = 1, LD_STREAM = 2, LD_COHERENT = 3, LD_CG = 4, LD_NA = 5 };
+__device__ __forceinline__ double2 ld_na(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ld_na(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ double2 ld_coherent(const double2* p) {
     double2 v;
     asm volatile("ld.relaxed.gpu.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
@@ -148,6 +159,8 @@ __device__ __forceinline__ float2 ld_coherent(const float2* p) {
 }
 template <class T, int LD> __device__ __forceinline__ typename V2<T>::type ldg2(const typename V2<T>::type* p) {
     if (LD == LD_COHERENT) return ld_coherent(p);
+    if (LD == LD_CG) return __ldcg(p);
+    if (LD == LD_NA) return ld_na(p);
     return LD == LD_RO ? __ldg(p) : (LD == LD_STREAM ? __ldcs(p) : *p);
 }
 template <class T, bool STREAM> __device__ __forceinline__ void stg2(typename V2<T>::type* p, typename V2<T>::type v) {

@@ -32,6 +32,7 @@ struct AuxArgs {
 #define SUG_DECLARE_NC(N)                                                                                   \
     cudaError_t update_nc##N(const Variant&, int kind, const UpdateArgs&, cudaStream_t, uint64_t* n_launch); \
     int update_spb_nc##N(const Variant&, int kind);                                                          \
+    long long update_coop_sites_nc##N(const Variant&, int kind);                                             \
     cudaError_t plaquette_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);           \
     cudaError_t polyakov_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);            \
     cudaError_t reunit_nc##N(const Variant&, const AuxArgs&, cudaStream_t, uint64_t* n_launch);              \

@@ -11,6 +11,8 @@
 // (z-chunk, t, z within chunk, y, x/2), so that the data first touched at t+1 is touched again
 // (at t and t-1) before 2 * Zc/Lz time slices of all planes have streamed through L2.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "su_device.cuh"
 #include "fused_schedule.h"
 
@@ -42,6 +44,11 @@ namespace sug {
 #define SUG_FUSED_STREAM 0
 #endif
 
+// how the plain (one sub-step per launch) register kernels load neighbour links: LD_RO (ld.global.nc), LD_CG, LD_NA, LD_STREAM
+#ifndef SUG_NEIGHBOUR_LD
+#define SUG_NEIGHBOUR_LD LD_RO
+#endif
+
 struct UpdateArgs {
     void* links;
     Geom g;
@@ -52,6 +59,7 @@ struct UpdateArgs {
     int reunit;                        // != 0: project the updated link back to SU(Nc) right before the store (Nc <= 4 register kernels)
     int pf_slices;                     // > 0: every warp asks L2 for the link tiles of its sites' positions this many time slices ahead
     int dyn_smem;                      // host side only: unused dynamic shared memory per block (caps the resident blocks per SM)
+    int coop_passes;                   // > 0: cooperative launch that runs this many whole passes (8 sub-steps each) with grid barriers
     uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
     unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
     // slab mode: link buffers of the slabs below / above in t (peer memory over NVLink, or this device). The
@@ -189,7 +197,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
     typedef Mat<NC, T, UNR> M;
     typedef cx<T> C;
     constexpr int NSUB = NC * (NC - 1) / 2;
-    constexpr int LDT = (LDN == LD_RO && SUG_TMINUS_STREAM) ? LD_STREAM : LDN;     // links of the time slice below
+    constexpr int LDT = (!FUSED && SUG_TMINUS_STREAM) ? LD_STREAM : LDN;     // links of the time slice below
     const unsigned cb = s.cb;
     const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
     // heatbath, register kernels: the directions of all subgroup draws are link-independent; evaluate them
@@ -417,7 +425,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
             site_of_thread(a.g, tix, a.parity, s);
             if (a.pf_slices > 0)
                 prefetch_slices_ahead<LinkIO<NC, T, STORE, UNR>::E, typename V2<T>::type>(a.links, a.g, __shfl_sync(warp_mask, s.cb, 0), a.pf_slices);
-            update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, LD_RO, PRE, false>(
+            update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, SUG_NEIGHBOUR_LD, PRE, false>(
                 a, a.parity, a.mu, s, tix, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
         }
     } else {
@@ -520,79 +528,75 @@ template <class T, int LD> __device__ __forceinline__ void qload(const typename 
 }
 template <class T> __device__ __forceinline__ void qconj(const T a[4], T o[4]) { o[0] = a[0]; o[1] = -a[1]; o[2] = -a[2]; o[3] = -a[3]; }
 
-template <class T, int KIND, int BLOCK, int MINB>
-__global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) {
+// one SU(2) link U_mu(x), x = s of parity p. LDN: how neighbour links are loaded; PLAIN: one sub-step per launch (streaming
+// own link, halo push in slab mode) - false inside the cooperative whole-pass kernel
+template <class T, int KIND, int LDN, bool PLAIN>
+__device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p, const int mu, const SiteNbr& s, const unsigned tix,
+                                                const unsigned warp_mask, const uint32_t sweep_ctr, unsigned& att_total, unsigned& exhausted) {
     typedef typename V2<T>::type T2;
-    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
-    const bool active = tix < a.g.Vh_int;
-    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);
-    unsigned att_total = 0, exhausted = 0;
-    if (active) {
-        const int p = a.parity, mu = a.mu;
-        SiteNbr s;
-        site_of_thread(a.g, tix, p, s);
-        const unsigned cb = s.cb;
-        const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
-        const T2* base = (const T2*)a.links;
-        auto plane = [&](int d, int par) { return base + (size_t)(d * 2 + par) * 2 * a.g.Vhp; };
-        T S[4] = {0, 0, 0, 0}, A[4], B[4], Cq[4], P[4], Q[4];
-        const T2* pl_mu_o = plane(mu, 1 - p);
+    const unsigned cb = s.cb;
+    const int dpmu = sel4(mu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+    const T2* base = (const T2*)a.links;
+    auto plane = [&](int d, int par) { return base + (size_t)(d * 2 + par) * 2 * a.g.Vhp; };
+    T S[4] = {0, 0, 0, 0}, A[4], B[4], Cq[4], P[4], Q[4];
+    const T2* pl_mu_o = plane(mu, 1 - p);
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int nu = k + (k >= mu ? 1 : 0);
-            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
-            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
-            const T2* pl_nu_s = plane(nu, p);
-            const T2* pl_nu_o = plane(nu, 1 - p);
-            qload<T, LD_RO>(pl_nu_s, cb, A);
-            qload<T, LD_RO>(pl_mu_o, cb + (unsigned)dpnu, B);
-            qload<T, LD_RO>(pl_nu_o, cb + (unsigned)dpmu, Cq);
-            quat_mul(A, B, P); qconj(Cq, A); quat_mul(P, A, Q);
-            S[0] += Q[0]; S[1] += Q[1]; S[2] += Q[2]; S[3] += Q[3];
-            qload<T, LD_RO>(pl_nu_o, cb + (unsigned)dmnu, A);
-            qload<T, LD_RO>(pl_mu_o, cb + (unsigned)dmnu, B);
-            qload<T, LD_RO>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), Cq);
-            qconj(A, P); quat_mul(P, B, Q); quat_mul(Q, Cq, P);
-            S[0] += P[0]; S[1] += P[1]; S[2] += P[2]; S[3] += P[3];
-        }
-        T2* pl_self = (T2*)a.links + (size_t)(mu * 2 + p) * 2 * a.g.Vhp;
-        T U[4], W[4], a4[4] = {1, 0, 0, 0};
-        qload<T, LD_STREAM>(pl_self, cb, U);
-        qconj(S, A);
-        quat_mul(U, A, W);
-        const T n2 = W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3];      // k^2
-        bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
-        int used = 0;
-        const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
-        if (ok) {
-            if (KIND == KIND_HB) {
-                const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;
-                T ud[4] = {W[0] * ik, -W[1] * ik, -W[2] * ik, -W[3] * ik};
-                T v[4];
-                used = kp_draw<T>(draw_mask, (T)a.beta * k, (T)-0.5 / (T)a.beta * ik, a.k0, a.k1, s.lex, a.sweep_ptr ? *a.sweep_ptr : a.sweep,
-                                  pack_c2((int)a.pass, p, mu, 0), v);
-                if (used) quat_mul(v, ud, a4); else ok = false;
-            } else {
-                // a = conj(W)^2 / k^2 (eq 17)
-                const T in2 = (T)1 / n2, m2w0 = (T)-2 * W[0] * in2;
-                a4[0] = (W[0] * W[0] - (W[1] * W[1] + W[2] * W[2] + W[3] * W[3])) * in2;
-                a4[1] = m2w0 * W[1]; a4[2] = m2w0 * W[2]; a4[3] = m2w0 * W[3];
-            }
-        }
+    for (int k = 0; k < 3; ++k) {
+        const int nu = k + (k >= mu ? 1 : 0);
+        const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+        const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+        const T2* pl_nu_s = plane(nu, p);
+        const T2* pl_nu_o = plane(nu, 1 - p);
+        qload<T, LDN>(pl_nu_s, cb, A);
+        qload<T, LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
+        qload<T, LDN>(pl_nu_o, cb + (unsigned)dpmu, Cq);
+        quat_mul(A, B, P); qconj(Cq, A); quat_mul(P, A, Q);
+        S[0] += Q[0]; S[1] += Q[1]; S[2] += Q[2]; S[3] += Q[3];
+        qload<T, LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
+        qload<T, LDN>(pl_mu_o, cb + (unsigned)dmnu, B);
+        qload<T, LDN>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), Cq);
+        qconj(A, P); quat_mul(P, B, Q); quat_mul(Q, Cq, P);
+        S[0] += P[0]; S[1] += P[1]; S[2] += P[2]; S[3] += P[3];
+    }
+    T2* pl_self = (T2*)a.links + (size_t)(mu * 2 + p) * 2 * a.g.Vhp;
+    T U[4], W[4], a4[4] = {1, 0, 0, 0};
+    qload<T, PLAIN ? LD_STREAM : LDN>(pl_self, cb, U);
+    qconj(S, A);
+    quat_mul(U, A, W);
+    const T n2 = W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3];      // k^2
+    bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
+    int used = 0;
+    const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
+    if (ok) {
         if (KIND == KIND_HB) {
-            att_total = (unsigned)used;
-            exhausted = ok ? 0u : 1u;
-            if (a.attempts) a.attempts[cb] = (uint8_t)(used > 255 ? 255 : used);
+            const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;
+            T ud[4] = {W[0] * ik, -W[1] * ik, -W[2] * ik, -W[3] * ik};
+            T v[4];
+            used = kp_draw<T>(draw_mask, (T)a.beta * k, (T)-0.5 / (T)a.beta * ik, a.k0, a.k1, s.lex, sweep_ctr,
+                              pack_c2((int)a.pass, p, mu, 0), v);
+            if (used) quat_mul(v, ud, a4); else ok = false;
+        } else {
+            // a = conj(W)^2 / k^2 (eq 17)
+            const T in2 = (T)1 / n2, m2w0 = (T)-2 * W[0] * in2;
+            a4[0] = (W[0] * W[0] - (W[1] * W[1] + W[2] * W[2] + W[3] * W[3])) * in2;
+            a4[1] = m2w0 * W[1]; a4[2] = m2w0 * W[2]; a4[3] = m2w0 * W[3];
         }
-        if (ok) {
-            quat_mul(a4, U, P);
-            if (a.reunit) {
-                const T inv = (T)1 / Fn<T>::sqrt(P[0] * P[0] + P[1] * P[1] + P[2] * P[2] + P[3] * P[3]);
-                P[0] *= inv; P[1] *= inv; P[2] *= inv; P[3] *= inv;
-            }
-            T2* q = pl_self + qsite<T>(cb);
-            stg2<T, true>(q, V2<T>::make(P[0], P[1]));
-            stg2<T, true>(q + LINK_TILE, V2<T>::make(P[2], P[3]));
+    }
+    if (KIND == KIND_HB) {
+        att_total += (unsigned)used;
+        exhausted += ok ? 0u : 1u;
+        if (a.attempts) a.attempts[cb] = (uint8_t)(used > 255 ? 255 : used);
+    }
+    if (ok) {
+        quat_mul(a4, U, P);
+        if (a.reunit) {
+            const T inv = (T)1 / Fn<T>::sqrt(P[0] * P[0] + P[1] * P[1] + P[2] * P[2] + P[3] * P[3]);
+            P[0] *= inv; P[1] *= inv; P[2] *= inv; P[3] *= inv;
+        }
+        T2* q = pl_self + qsite<T>(cb);
+        stg2<T, PLAIN>(q, V2<T>::make(P[0], P[1]));
+        stg2<T, PLAIN>(q + LINK_TILE, V2<T>::make(P[2], P[3]));
+        if (PLAIN) {
             if (const int edge = slab_edge(a.g, tix)) {      // fused halo push (slab mode only)
                 const size_t plane_off = (size_t)(mu * 2 + p) * 2 * a.g.Vhp;
                 if (edge & 1) {
@@ -606,16 +610,98 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
             }
         }
     }
-    if (KIND == KIND_HB) {
-        for (int o = 16; o > 0; o >>= 1) {
-            att_total += __shfl_down_sync(0xffffffffu, att_total, o);
-            exhausted += __shfl_down_sync(0xffffffffu, exhausted, o);
-        }
-        if ((threadIdx.x & 31) == 0) {
-            if (att_total) atomicAdd(a.counters, (unsigned long long)att_total);
-            if (exhausted) atomicAdd(a.counters + 1, (unsigned long long)exhausted);
+}
+
+__device__ __forceinline__ void flush_kp_counters(const UpdateArgs& a, unsigned att_total, unsigned exhausted) {
+    for (int o = 16; o > 0; o >>= 1) {
+        att_total += __shfl_down_sync(0xffffffffu, att_total, o);
+        exhausted += __shfl_down_sync(0xffffffffu, exhausted, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (att_total) atomicAdd(a.counters, (unsigned long long)att_total);
+        if (exhausted) atomicAdd(a.counters + 1, (unsigned long long)exhausted);
+    }
+}
+
+template <class T, int KIND, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) {
+    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tix < a.g.Vh_int;
+    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);
+    unsigned att_total = 0, exhausted = 0;
+    if (active) {
+        SiteNbr s;
+        site_of_thread(a.g, tix, a.parity, s);
+        update_link_su2<T, KIND, LD_RO, true>(a, a.parity, a.mu, s, tix, warp_mask, a.sweep_ptr ? *a.sweep_ptr : a.sweep, att_total, exhausted);
+    }
+    if (KIND == KIND_HB) flush_kp_counters(a, att_total, exhausted);
+}
+
+// ------------------------------------------------------------------------------------------
+// Cooperative whole-pass kernels (su_set_option "coop_sweep"; SURVEY.md 7 "small lattices are launch-bound"): when all
+// the blocks of a sub-step fit the device at once, ONE cooperative launch runs a.coop_passes whole passes - 8 sub-steps
+// each, in the order of reading R6 - with a grid barrier in place of every launch boundary. Same threads, same sites,
+// same arithmetic as the plain launches (bitwise equal); neighbour links are read with ld.global.cg (L2 only), which
+// needs no L1 invalidation to see what other blocks stored before the barrier. a.pass = number of the first pass;
+// a.reunit applies to the last pass of the launch. Not for slab handles (no halo push in here).
+// ------------------------------------------------------------------------------------------
+template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, int FUSE3 = 0, bool KUNR = false>
+__global__ void __launch_bounds__(BLOCK, MINB) k_update_coop(const UpdateArgs a) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    constexpr int NSUB = NC * (NC - 1) / 2;
+    constexpr int PRE_ASKED = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
+    constexpr int PRE = (PRE_ASKED == 4 && !FUSE3) ? (sizeof(T) == 4 ? 1 : 0) : PRE_ASKED;
+    __shared__ T dir_sm[PRE >= 2 ? 5 * NSUB : (PRE == 1 ? 3 * NSUB : 1)][PRE ? BLOCK : 1];
+    const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
+    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tix < a.g.Vh_int;
+    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);
+    unsigned att_total = 0, exhausted = 0;
+    UpdateArgs b = a;
+#pragma unroll 1
+    for (int ps = 0; ps < a.coop_passes; ++ps) {
+        b.pass = a.pass + (uint32_t)ps;
+        b.reunit = (a.reunit && ps == a.coop_passes - 1) ? 1 : 0;
+#pragma unroll 1
+        for (int sub = 0; sub < 8; ++sub) {
+            if (active) {
+                SiteNbr s;
+                site_of_thread(a.g, tix, sub >> 2, s);
+                update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, LD_CG, PRE, true>(
+                    b, sub >> 2, sub & 3, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
+            }
+            grid.sync();
         }
     }
+    if (KIND == KIND_HB) flush_kp_counters(a, att_total, exhausted);
+}
+
+template <class T, int KIND, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) k_update_su2_coop(const UpdateArgs a) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
+    const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
+    const bool active = tix < a.g.Vh_int;
+    const unsigned warp_mask = __ballot_sync(0xffffffffu, active);
+    unsigned att_total = 0, exhausted = 0;
+    UpdateArgs b = a;
+#pragma unroll 1
+    for (int ps = 0; ps < a.coop_passes; ++ps) {
+        b.pass = a.pass + (uint32_t)ps;
+        b.reunit = (a.reunit && ps == a.coop_passes - 1) ? 1 : 0;
+#pragma unroll 1
+        for (int sub = 0; sub < 8; ++sub) {
+            if (active) {
+                SiteNbr s;
+                site_of_thread(a.g, tix, sub >> 2, s);
+                update_link_su2<T, KIND, LD_CG, false>(b, sub >> 2, sub & 3, s, tix, warp_mask, sweep_ctr, att_total, exhausted);
+            }
+            grid.sync();
+        }
+    }
+    if (KIND == KIND_HB) flush_kp_counters(a, att_total, exhausted);
 }
 
 }  // namespace sug

@@ -13,6 +13,7 @@
 
 namespace sug {
 
+constexpr int NC_ = SUG_NC;
 #define SUG_CAT_(a, b) a##b
 #define SUG_CAT(a, b) SUG_CAT_(a, b)
 
@@ -38,10 +39,27 @@ template <class K> static void launch_k(K kern, unsigned grid, int block, cudaSt
     kern<<<grid, block, a.dyn_smem, st>>>(a);
 }
 
+// cooperative whole-pass launch (k_update_coop): every block of a sub-step resident at once, grid barriers inside
+template <class K> static cudaError_t launch_coop(K kern, unsigned grid, int block, cudaStream_t st, const UpdateArgs& a) {
+    void* args[] = {(void*)&a};
+    return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(block), args, 0, st);
+}
+// sites of one parity that a cooperative launch of this kernel can hold (0: cannot be queried)
+template <class K> static long long coop_capacity(K kern, int block) {
+    int dev = 0, sms = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, block, 0) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return (long long)per_sm * sms * block;
+}
+
 // a.fz.work != NULL: the fused launch of a.fz.fg.g consecutive sub-steps (fused_schedule.h), one block per ticket
 template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB>
 static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t st) {
     const bool fused = a.fz.work != nullptr;
+    if (a.coop_passes > 0) {
+        if (kind == KIND_HB) return launch_coop(k_update_coop<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR>, (a.g.Vh_int + HB::BLOCK - 1) / HB::BLOCK, HB::BLOCK, st, a);
+        return launch_coop(k_update_coop<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR>, (a.g.Vh_int + OR::BLOCK - 1) / OR::BLOCK, OR::BLOCK, st, a);
+    }
     if (kind == KIND_HB) {
         const unsigned grid = (a.g.Vh_int + HB::BLOCK - 1) / HB::BLOCK;
         if (fused) launch_k(k_update<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR, true>, a.fz.n_tickets, HB::BLOCK, st, a);
@@ -54,6 +72,10 @@ static cudaError_t launch_update_t(int kind, const UpdateArgs& a, cudaStream_t s
     return cudaGetLastError();
 }
 template <class HB, class OR = HB> static int spb_t(int kind) { return kind == KIND_HB ? HB::BLOCK : OR::BLOCK; }
+template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB> static long long coop_sites_t(int kind) {
+    if (kind == KIND_HB) return coop_capacity(k_update_coop<NC, T, STORE, KIND_HB, UNR, HB::BLOCK, HB::MINB, HB::FUSE3, HB::KUNR>, HB::BLOCK);
+    return coop_capacity(k_update_coop<NC, T, STORE, KIND_OR, UNR, OR::BLOCK, OR::MINB, OR::FUSE3, OR::KUNR>, OR::BLOCK);
+}
 
 // Tuning overrides (-DSUG_CFG_...="Cfg<...>"), used only while sweeping on the GPU; the defaults below are
 // the measured choices (profiles/).
@@ -66,11 +88,15 @@ template <class HB, class OR = HB> static int spb_t(int kind) { return kind == K
 #ifndef SUG_SU3_F64_SMODE
 #define SUG_SU3_F64_SMODE 1
 #endif
+// heatbath, fp64: 2 blocks of 192 threads (the same 12 warps per SM as 3 x 128) measured 2-3 % faster (profiles/r02g)
 #ifndef SUG_SU3_F64_HB_MINB
-#define SUG_SU3_F64_HB_MINB SUG_SU3_F64_MINB
+#define SUG_SU3_F64_HB_MINB 2
+#endif
+#ifndef SUG_SU3_F64_HB_BLOCK
+#define SUG_SU3_F64_HB_BLOCK 192
 #endif
 #ifndef SUG_CFG_SU3_F64_HB
-#define SUG_CFG_SU3_F64_HB Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_HB_MINB, SUG_SU3_F64_SMODE, true>
+#define SUG_CFG_SU3_F64_HB Cfg<SUG_SU3_F64_HB_BLOCK, SUG_SU3_F64_HB_MINB, SUG_SU3_F64_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3_F64_OR
 #define SUG_CFG_SU3_F64_OR Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, SUG_SU3_F64_SMODE, true>
@@ -130,6 +156,10 @@ cudaError_t SUG_CAT(update_nc, SUG_NC)(const Variant& v, int kind, const UpdateA
     if (!v.generic) {
         constexpr int BLOCK = 128;
         const unsigned grid = (a.g.Vh_int + BLOCK - 1) / BLOCK;
+        if (a.coop_passes > 0) {
+            if (f64) return kind == KIND_HB ? launch_coop(k_update_su2_coop<double, KIND_HB, BLOCK, 4>, grid, BLOCK, st, a) : launch_coop(k_update_su2_coop<double, KIND_OR, BLOCK, 4>, grid, BLOCK, st, a);
+            return kind == KIND_HB ? launch_coop(k_update_su2_coop<float, KIND_HB, BLOCK, 4>, grid, BLOCK, st, a) : launch_coop(k_update_su2_coop<float, KIND_OR, BLOCK, 4>, grid, BLOCK, st, a);
+        }
         if (f64) { if (kind == KIND_HB) k_update_su2<double, KIND_HB, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); else k_update_su2<double, KIND_OR, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); }
         else     { if (kind == KIND_HB) k_update_su2<float,  KIND_HB, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); else k_update_su2<float,  KIND_OR, BLOCK, 4><<<grid, BLOCK, 0, st>>>(a); }
         return cudaGetLastError();
@@ -177,6 +207,31 @@ int SUG_CAT(update_spb_nc, SUG_NC)(const Variant& v, int kind) {
     return 0;
 #else
     (void)f64;
+    return 0;
+#endif
+}
+
+// Sites of one parity that fit ONE cooperative whole-pass launch of the kernel update_nc would use for this variant and
+// kind (all blocks resident at once); 0: this kernel has no cooperative form.
+long long SUG_CAT(update_coop_sites_nc, SUG_NC)(const Variant& v, int kind) {
+    const bool f64 = v.prec == SU_FP64;
+#if SUG_NC == 2
+    if (v.generic) return 0;
+    if (f64) return kind == KIND_HB ? coop_capacity(k_update_su2_coop<double, KIND_HB, 128, 4>, 128) : coop_capacity(k_update_su2_coop<double, KIND_OR, 128, 4>, 128);
+    return kind == KIND_HB ? coop_capacity(k_update_su2_coop<float, KIND_HB, 128, 4>, 128) : coop_capacity(k_update_su2_coop<float, KIND_OR, 128, 4>, 128);
+#elif SUG_NC == 3
+    if (v.generic) return 0;
+    if (v.store == STORE_RECON12)
+        return f64 ? coop_sites_t<NC_, double, STORE_RECON12, true, SUG_CFG_SU3R_F64_HB, SUG_CFG_SU3R_F64_OR>(kind)
+                   : coop_sites_t<NC_, float,  STORE_RECON12, true, SUG_CFG_SU3R_F32_HB, SUG_CFG_SU3R_F32_OR>(kind);
+    return f64 ? coop_sites_t<NC_, double, STORE_FULL, true, SUG_CFG_SU3_F64_HB, SUG_CFG_SU3_F64_OR>(kind)
+               : coop_sites_t<NC_, float,  STORE_FULL, true, SUG_CFG_SU3_F32_HB, SUG_CFG_SU3_F32_OR>(kind);
+#elif SUG_NC == 4
+    if (v.generic) return 0;
+    return f64 ? coop_sites_t<NC_, double, STORE_FULL, true, SUG_CFG_SU4_F64_HB, SUG_CFG_SU4_F64_OR>(kind)
+               : coop_sites_t<NC_, float,  STORE_FULL, true, SUG_CFG_SU4_F32_HB, SUG_CFG_SU4_F32_OR>(kind);
+#else
+    (void)f64; (void)kind; (void)v;
     return 0;
 #endif
 }

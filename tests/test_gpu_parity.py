@@ -513,3 +513,95 @@ def test_reunitarise_on_store(mods, v):
     H0.sweep(BETA[Nc], 0, 1)
     out = H0.export_links()
     assert H.unitarity_defect(out) < tol_group
+
+
+@pytest.mark.parametrize("v", [(3, "fp64", False, "auto"), (3, "fp32", False, "auto"), (3, "fp64", True, "auto"),
+                               (4, "fp32", False, "auto")], ids=_ids)
+@pytest.mark.parametrize("dims", [(16, 8, 4, 6), (16, 16, 8, 4)], ids=lambda d: "x".join(map(str, d)))
+def test_traversal_and_prefetch_knobs_are_bitwise_neutral(mods, v, dims):
+    """su_set_option "block_tile_z" / "block_tile_t" (the warps of a block share x-y segments of neighbouring z-planes /
+    time slices), "prefetch_slices" (L2 bulk prefetch ahead of the traversal) and "blocks_per_sm" (occupancy cap) only
+    change which thread works on which site and what L2 is asked for early: sweeps, reunitarisation and the attempt
+    counters must be BITWISE those of the default traversal, also where the tile does not fit and is dropped."""
+    su, _ = mods
+    Nc, precision, recon12, kernel = v
+
+    def run(opts):
+        G = su.Lattice(Nc, dims, precision, recon12, kernel)
+        for k, val in opts.items():
+            G.set_option(k, val)
+            assert G.get_option(k) == val
+        G.init_hot(9)
+        for _ in range(2):
+            G.sweep(BETA[Nc], 1, 2)
+            G.reunitarize()
+        return G.export_links(), G.counters()
+
+    ref = run({})
+    for opts in ({"block_tile_z": 2, "block_tile_t": 2}, {"block_tile_z": 4}, {"block_tile_t": 2}, {"block_tile_z": 2, "z_chunk_planes": 2},
+                 {"prefetch_slices": 1}, {"prefetch_slices": 3, "block_tile_z": 2}, {"blocks_per_sm": 2}):
+        got = run(opts)
+        assert np.array_equal(got[0], ref[0]), opts
+        assert got[1] == ref[1], opts
+    G = su.Lattice(Nc, dims, precision, recon12, kernel)
+    for name, bad in (("block_tile_z", 0), ("block_tile_t", 9), ("prefetch_slices", -1), ("blocks_per_sm", 65)):
+        with pytest.raises(su.SuError):
+            G.set_option(name, bad)
+
+
+def test_measured_peaks_are_plausible(mods):
+    """su_measure_fma_peak / su_measure_l2_peak: the two micro-benchmarks behind the "alu" and "l2" roofs of bench.py."""
+    su, _ = mods
+    tf64, _ = su.measure_fma_peak("fp64")
+    tf32, _ = su.measure_fma_peak("fp32")
+    gbs, ms, bpc = su.measure_l2_peak()
+    assert 5.0 < tf64 < 100.0 and tf64 < tf32 < 200.0
+    assert 2000.0 < gbs < 40000.0 and ms > 0 and 1000.0 < bpc < 20000.0
+
+
+@pytest.mark.parametrize("v", [(2, "fp64", False, "auto"), (2, "fp32", False, "auto"), (3, "fp64", False, "auto"), (3, "fp32", False, "auto"),
+                               (3, "fp64", True, "auto"), (3, "fp32", True, "auto"), (4, "fp64", False, "auto"), (4, "fp32", False, "auto")], ids=_ids)
+@pytest.mark.parametrize("dims", [DIMS_ANISO, (8, 8, 8, 8)], ids=lambda d: "x".join(map(str, d)))
+def test_cooperative_whole_pass_launches_are_bitwise_the_plain_sweep(mods, v, dims):
+    """su_set_option("coop_sweep", 1): all heatbath passes of a sweep in one cooperative launch and all overrelaxation
+    passes in another, grid barriers instead of launch boundaries (small lattices are launch-bound). Same threads, same
+    sites, same arithmetic: links, attempt counters and plaquette must be BITWISE those of the 8 (n_hb + n_or) plain
+    launches, with two heatbath passes (pass number in the RNG counter), reunitarise-on-store and graph replay."""
+    su, _ = mods
+    Nc, precision, recon12, kernel = v
+
+    def run(coop, graph, reunit):
+        G = su.Lattice(Nc, dims, precision, recon12, kernel)
+        G.set_option("coop_sweep", coop)
+        if Nc > 2:
+            G.set_option("reunit_on_store", reunit)
+        G.init_hot(13)
+        n0 = G.launch_count()
+        if graph:
+            G.set_graph_mode(True)
+        for _ in range(3):
+            G.sweep(BETA[Nc], 2, 3)
+        n = G.launch_count() - n0
+        return G.export_links(), G.counters(), G.plaquette(), n, G.get_option("coop_sweep_effective")
+
+    for reunit in (0, 1):
+        ref = run(0, False, reunit)
+        assert ref[4] == 0
+        for graph in (False, True):
+            got = run(1, graph, reunit)
+            assert got[4] == 3                                   # both kinds fit the device at these sizes
+            assert np.array_equal(got[0], ref[0]), (graph, reunit)
+            assert got[1] == ref[1] and got[2] == ref[2]
+            assert got[3] <= 3 * 3, got[3]                       # two launches per sweep (+ the graph's counter node) instead of 40
+
+
+def test_cooperative_launch_falls_back_when_the_lattice_does_not_fit(mods):
+    su, _ = mods
+    G = su.Lattice(3, (32, 32, 32, 32), "fp64")                  # 524288 sites per parity: far more than one wave of blocks
+    G.set_option("coop_sweep", 1)
+    assert G.get_option("coop_sweep_effective") == 0
+    G.init_cold(1)
+    n0 = G.launch_count()
+    G.sweep(6.0, 1, 1)
+    assert G.launch_count() - n0 == 16
+    assert abs(G.plaquette() - 1.0) > 1e-3
