@@ -564,12 +564,24 @@ __device__ __forceinline__ int kp_draw(unsigned draw_mask, T alpha, T m_inv2a, u
     return used;
 }
 
+// Explicitly fused / unfused scalar operations. Where an expression a b + c d leaves the compiler a choice of which
+// product to fuse, two instances of the same source (plain, fused and cooperative kernels) can round differently in
+// the last bit; the few such expressions of the update are written with these so that every instance is bitwise the same.
+__device__ __forceinline__ float  fma_x(float a, float b, float c)    { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_x(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float  mul_x(float a, float b)   { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_x(double a, double b) { return __dmul_rn(a, b); }
+// a0^2 + a1^2 + a2^2 + a3^2, summed left to right
+template <class T> __device__ __forceinline__ T norm2_4(T a0, T a1, T a2, T a3) {
+    return fma_x(a3, a3, fma_x(a2, a2, fma_x(a1, a1, mul_x(a0, a0))));
+}
+
 // quaternion product, U = a0 + i a.sigma (eq 6): (ab)_0 = a0 b0 - a.b, (ab)_vec = a0 b + b0 a - a x b
 template <class T> __device__ __forceinline__ void quat_mul(const T a[4], const T b[4], T o[4]) {
-    o[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
-    o[1] = a[0] * b[1] + b[0] * a[1] - (a[2] * b[3] - a[3] * b[2]);
-    o[2] = a[0] * b[2] + b[0] * a[2] - (a[3] * b[1] - a[1] * b[3]);
-    o[3] = a[0] * b[3] + b[0] * a[3] - (a[1] * b[2] - a[2] * b[1]);
+    o[0] = fma_x(-a[3], b[3], fma_x(-a[2], b[2], fma_x(-a[1], b[1], mul_x(a[0], b[0]))));
+    o[1] = fma_x(a[3], b[2], fma_x(-a[2], b[3], fma_x(b[0], a[1], mul_x(a[0], b[1]))));
+    o[2] = fma_x(a[1], b[3], fma_x(-a[3], b[1], fma_x(b[0], a[2], mul_x(a[0], b[2]))));
+    o[3] = fma_x(a[2], b[1], fma_x(-a[1], b[2], fma_x(b[0], a[3], mul_x(a[0], b[3]))));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -596,7 +608,7 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
             const cx<T> wii = W[i * NC + i], wij = W[i * NC + j], wji = W[j * NC + i], wjj = W[j * NC + j];
             T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
             T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
-            const T n2 = r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3;          // k^2
+            const T n2 = norm2_4(r0, r1, r2, r3);                        // k^2
             bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
             T a[4] = {(T)1, (T)0, (T)0, (T)0};
             int used = 0;
@@ -613,7 +625,7 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                 } else {
                     // a = (u~^dagger)^2 = conj(r)^2 / k^2 (eq 17): no square root, one reciprocal
                     const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
-                    a[0] = (r0 * r0 - (r1 * r1 + r2 * r2 + r3 * r3)) * in2;
+                    a[0] = fma_x(r0, r0, -fma_x(r3, r3, fma_x(r2, r2, mul_x(r1, r1)))) * in2;
                     a[1] = m2r0 * r1; a[2] = m2r0 * r2; a[3] = m2r0 * r3;
                 }
             }

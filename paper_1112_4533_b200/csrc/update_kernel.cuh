@@ -563,7 +563,7 @@ __device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p
     qload<T, PLAIN ? LD_STREAM : LDN>(pl_self, cb, U);
     qconj(S, A);
     quat_mul(U, A, W);
-    const T n2 = W[0] * W[0] + W[1] * W[1] + W[2] * W[2] + W[3] * W[3];      // k^2
+    const T n2 = norm2_4(W[0], W[1], W[2], W[3]);      // k^2
     bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
     int used = 0;
     const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
@@ -578,7 +578,7 @@ __device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p
         } else {
             // a = conj(W)^2 / k^2 (eq 17)
             const T in2 = (T)1 / n2, m2w0 = (T)-2 * W[0] * in2;
-            a4[0] = (W[0] * W[0] - (W[1] * W[1] + W[2] * W[2] + W[3] * W[3])) * in2;
+            a4[0] = fma_x(W[0], W[0], -fma_x(W[3], W[3], fma_x(W[2], W[2], mul_x(W[1], W[1])))) * in2;
             a4[1] = m2w0 * W[1]; a4[2] = m2w0 * W[2]; a4[3] = m2w0 * W[3];
         }
     }
@@ -590,7 +590,7 @@ __device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p
     if (ok) {
         quat_mul(a4, U, P);
         if (a.reunit) {
-            const T inv = (T)1 / Fn<T>::sqrt(P[0] * P[0] + P[1] * P[1] + P[2] * P[2] + P[3] * P[3]);
+            const T inv = (T)1 / Fn<T>::sqrt(norm2_4(P[0], P[1], P[2], P[3]));
             P[0] *= inv; P[1] *= inv; P[2] *= inv; P[3] *= inv;
         }
         T2* q = pl_self + qsite<T>(cb);
