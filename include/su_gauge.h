@@ -196,7 +196,8 @@ su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* o
  *                     sweep (tested). Measured no faster than the CUDA-graph replay of the 40 launches (profiles/r02g).
  *   "block_tile_z", "block_tile_t"   the warps of a thread block of the Nc = 3, 4 register kernels work on the same x-y
  *                     segments of this many consecutive z-planes / time slices (1: a block is consecutive segments of
- *                     one plane), dropped silently where the lattice or the block does not divide evenly.
+ *                     one plane), dropped silently where the lattice or the block does not divide evenly. Only in libraries built
+ *                     with -DSUG_BLOCK_TILES=1 (su_get_option "block_tiles_supported"); otherwise values != 1: SU_EUNSUPPORTED.
  *   "prefetch_slices" k > 0: every warp of an update kernel asks L2 (cp.async.bulk.prefetch.L2) for the link tiles of
  *                     its sites' positions k time slices ahead of the traversal. A hint; 0 (default) = off.
  *   "blocks_per_sm"   n > 0: update launches request unused dynamic shared memory so that only n blocks fit an SM.
@@ -231,6 +232,11 @@ su_status su_measure_fma_peak(int device, su_precision p, double* tflops, double
  * ms (may be NULL): duration of the best launch; bytes_per_clock (may be NULL): the same throughput per SM clock
  * cycle (clock64 span of one block), the figure that carries over to a run at another clock. Synchronises the device. */
 su_status su_measure_l2_peak(int device, int through_l1, double* gbs, double* ms, double* bytes_per_clock);
+
+/* Test hook: the elementary functions of the Kennedy-Pendleton draw exactly as the fp64 kernels evaluate them (branch-free
+ * ln / sincos / sqrt / rsqrt of csrc/su_device.cuh). For each of the n host words w, u = (w + 1) / 2^32:
+ * out[5 i + 0..4] = ln u, sin 2 pi u, cos 2 pi u, sqrt u, 1 / sqrt(100 u + 0.001). Host pointers; synchronises. */
+su_status su_debug_kp_math(int device, const uint32_t* words, size_t n, double* out);
 
 /* Text of the last error on this handle ("" if none); static text if the handle is NULL.
  * Owned by the library, valid until the next call on the handle. */

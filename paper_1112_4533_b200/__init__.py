@@ -32,7 +32,7 @@ ABI_SYMBOLS = (
     "su_synchronize", "su_set_graph_mode", "su_set_timing", "su_get_timing", "su_get_launch_count", "su_last_error",
     "su_lattice_create_slab", "su_slab_bytes", "su_slab_links", "su_slab_set_peers", "su_slab_halo_push",
     "su_ipc_export", "su_ipc_open", "su_ipc_close", "su_slab_plaquette_sum", "su_set_option", "su_get_option",
-    "su_measure_fma_peak", "su_measure_l2_peak", "su_save_config", "su_load_config", "su_fused_schedule_debug", "su_fused_dep_debug",
+    "su_measure_fma_peak", "su_measure_l2_peak", "su_debug_kp_math", "su_save_config", "su_load_config", "su_fused_schedule_debug", "su_fused_dep_debug",
 )
 
 
@@ -98,6 +98,7 @@ def lib():
     L.su_save_config.argtypes = [P, C.c_char_p]
     L.su_load_config.argtypes = [P, C.c_char_p]
     L.su_measure_fma_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D)]
+    L.su_debug_kp_math.argtypes = [I, C.c_void_p, C.c_size_t, C.c_void_p]
     L.su_measure_l2_peak.argtypes = [I, I, C.POINTER(D), C.POINTER(D), C.POINTER(D)]
     L.su_set_option.argtypes = [P, C.c_char_p, C.c_longlong]
     L.su_get_option.argtypes = [P, C.c_char_p, C.POINTER(C.c_longlong)]
@@ -127,6 +128,17 @@ def measure_fma_peak(precision="fp64", device=-1):
     if st != SU_OK:
         raise SuError(st, "su_measure_fma_peak")
     return t.value, ms.value
+
+
+def debug_kp_math(words, device=-1):
+    """-> array [n, 5]: ln u, sin 2 pi u, cos 2 pi u, sqrt u, 1 / sqrt(100 u + 0.001) for u = (w + 1) / 2^32 (su_debug_kp_math)"""
+    import numpy as np
+    w = np.ascontiguousarray(words, dtype=np.uint32)
+    out = np.empty((w.size, 5), dtype=np.float64)
+    st = lib().su_debug_kp_math(device, w.ctypes.data, w.size, out.ctypes.data)
+    if st != SU_OK:
+        raise SuError(st, "su_debug_kp_math")
+    return out
 
 
 def measure_l2_peak(device=-1, through_l1=False):

@@ -207,7 +207,7 @@ __global__ void k_update_big(const UpdateArgs a, const BigCommon bc) {
         const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(0xffffffffu, ok) : 0u;
         if (ok) {
             if (KIND == KIND_HB) {
-                const T ik = Fn<T>::rsqrt(n2), kk = n2 * ik;
+                const T ik = Fn<T>::rsqrt_pos(n2), kk = n2 * ik;
                 T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                 T v[4];
                 used = kp_draw<T>(draw_mask, two_beta_over_nc * kk, m_nc_over_4beta * ik, a.k0, a.k1, s.lex, c1, c2_base | (uint32_t)sub, v);

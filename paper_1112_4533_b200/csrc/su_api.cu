@@ -199,6 +199,20 @@ __global__ void __launch_bounds__(256) k_l2_peak(double* out, const double2* __r
     if (blockIdx.x == 0 && threadIdx.x == 0) out[0] = (double)(clock64() - c0);     // SM clocks of a block that ran start to end
 }
 
+// su_debug_kp_math: the elementary functions of the Kennedy-Pendleton draw as the fp64 kernels evaluate them
+__global__ void k_debug_kp_math(const uint32_t* w, size_t n, double* out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double u = ((double)w[i] + 1.0) * (1.0 / 4294967296.0);
+    double sn, cs;
+    Fn<double>::sincos2pi_w(w[i], &sn, &cs);
+    out[5 * i + 0] = Fn<double>::log_w(w[i]);
+    out[5 * i + 1] = sn;
+    out[5 * i + 2] = cs;
+    out[5 * i + 3] = Fn<double>::sqrt01(u);
+    out[5 * i + 4] = Fn<double>::rsqrt_pos(100.0 * u + 1e-3);
+}
+
 void free_fused(su_lattice* h) {
     for (auto& kv : h->fused) {
         cudaFree(kv.second.d_work); cudaFree(kv.second.d_done); cudaFree(kv.second.d_ctrl);
@@ -991,6 +1005,7 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
     }
     if (!strcmp(name, "block_tile_z") || !strcmp(name, "block_tile_t")) {
         if (value < 1 || value > 8) return fail(h, SU_EINVAL, "%s must be in 1...8", name);
+        if (!SUG_BLOCK_TILES && value != 1) return fail(h, SU_EUNSUPPORTED, "%s: this library was built without -DSUG_BLOCK_TILES=1", name);
         SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
         free_graphs(h);
         (name[11] == 'z' ? h->tile_z : h->tile_t) = (int)value;
@@ -1028,6 +1043,7 @@ su_status su_get_option(su_lattice* h, const char* name, long long* value) {
     if (!strcmp(name, "reunit_on_store")) { *value = h->reunit_on_store ? 1 : 0; return SU_OK; }
     if (!strcmp(name, "coop_sweep")) { *value = h->coop_sweep ? 1 : 0; return SU_OK; }
     if (!strcmp(name, "coop_sweep_effective")) { *value = (coop_fits(h, 0) ? 1 : 0) | (coop_fits(h, 1) ? 2 : 0); return SU_OK; }
+    if (!strcmp(name, "block_tiles_supported")) { *value = SUG_BLOCK_TILES; return SU_OK; }
     if (!strcmp(name, "block_tile_z")) { *value = h->tile_z; return SU_OK; }
     if (!strcmp(name, "block_tile_t")) { *value = h->tile_t; return SU_OK; }
     if (!strcmp(name, "prefetch_slices")) { *value = h->prefetch_slices; return SU_OK; }
@@ -1136,6 +1152,26 @@ su_status su_measure_l2_peak(int device, int through_l1, double* gbs, double* ms
     if (ms) *ms = best;
     if (bytes_per_clock) *bytes_per_clock = clocks > 0 ? per_block * blocks / clocks : 0.0;
     return SU_OK;
+}
+
+su_status su_debug_kp_math(int device, const uint32_t* words, size_t n, double* out) {
+    if (!words || !out || n == 0) return SU_EINVAL;
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return SU_ECUDA;
+    DeviceGuard guard(dev);
+    uint32_t* d_w = nullptr;
+    double* d_o = nullptr;
+    su_status st = SU_OK;
+    if (cudaMalloc(&d_w, n * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&d_o, n * 5 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
+    if (st == SU_OK) {
+        cudaMemcpy(d_w, words, n * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        k_debug_kp_math<<<(unsigned)((n + 255) / 256), 256>>>(d_w, n, d_o);
+        if (cudaMemcpy(out, d_o, n * 5 * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) st = SU_ECUDA;
+    }
+    if (d_w) cudaFree(d_w);
+    if (d_o) cudaFree(d_o);
+    if (st != SU_OK) cudaGetLastError();
+    return st;
 }
 
 const char* su_last_error(const su_lattice* h) { return h ? h->err : kNullHandle; }

@@ -442,6 +442,98 @@ __device__ __forceinline__ uint32_t pack_c2(int pass, int parity, int mu, int su
 }
 __device__ __forceinline__ uint32_t c2_kind(uint32_t c2_low, int kind) { return c2_low | ((uint32_t)kind << 28); }
 
+// ------------------------------------------------------------------------------------------
+// Branch-free fp64 elementary functions for the Kennedy-Pendleton draw (-DSUG_FAST_MATH64=0: libdevice instead).
+// The draw needs ln u, cos 2 pi u, sincos 2 pi u for u = (w + 1) / 2^32 with w a 32-bit Philox word, and square roots
+// of numbers in [0, 1] / positive norms: no special cases, so no branches or slow-path calls - libdevice's versions
+// carry both, which keeps the compiler from interleaving the chains of independent draws with each other or with loads
+// (profiles/r02a, r02g). Accuracy <= 1 ulp-level (2.2e-16 relative for ln, 1.8e-16 absolute for sin / cos: checked against
+// long double on 2^24 words and the edge words by tests/test_gpu_parity.py::test_fast_math_against_host).
+// ------------------------------------------------------------------------------------------
+#ifndef SUG_FAST_MATH64
+#define SUG_FAST_MATH64 1
+#endif
+__device__ __forceinline__ double rcp_approx64(double x) { double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x)); return r; }
+__device__ __forceinline__ double rsqrt_approx64(double x) { double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x)); return r; }
+
+// ln((w + 1) / 2^32): n = w + 1 = m 2^e with m in [sqrt(1/2), sqrt 2], ln m = 2 atanh(s), s = (m - 1) / (m + 1), by its
+// Taylor series to s^21 (|s| <= 0.172: next term 2e-17 relative), the division by a Newton-refined reciprocal.
+__device__ __forceinline__ double fast_log_u01(uint32_t w) {
+    const double n = (__hiloint2double(0x43300000, (int)w) - 4503599627370496.0) + 1.0;      // exact: 1 ... 2^32
+    const int hi = __double2hiint(n), lo = __double2loint(n);
+    int e = (hi >> 20) - 1023;
+    int mh = (hi & 0x000fffff) | 0x3ff00000;
+    const int big = mh > 0x3ff6a09e ? 1 : 0;                        // m > sqrt 2 (to 2^-20): halve it
+    mh -= big << 20; e += big;
+    const double f = __hiloint2double(mh, lo) - 1.0, d = 2.0 + f;
+    double r = rcp_approx64(d);
+    r = __fma_rn(r, __fma_rn(-d, r, 1.0), r);
+    r = __fma_rn(r, __fma_rn(-d, r, 1.0), r);
+    double sq = f * r;
+    sq = __fma_rn(__fma_rn(-d, sq, f), r, sq);
+    const double z = sq * sq;
+    double P = 0.09523809523809523;                                 // 2 / 21
+    P = __fma_rn(P, z, 0.10526315789473684);
+    P = __fma_rn(P, z, 0.11764705882352941);
+    P = __fma_rn(P, z, 0.13333333333333333);
+    P = __fma_rn(P, z, 0.15384615384615385);
+    P = __fma_rn(P, z, 0.18181818181818182);
+    P = __fma_rn(P, z, 0.2222222222222222);
+    P = __fma_rn(P, z, 0.2857142857142857);
+    P = __fma_rn(P, z, 0.4);
+    P = __fma_rn(P, z, 0.6666666666666666);
+    const double k = (double)(e - 32);
+    // k ln2_hi is exact (ln2_hi has 32 trailing zero bits)
+    return __fma_rn(k, 6.93147180369123816490e-01, __fma_rn(2.0, sq, __fma_rn(sq * z, P, k * 1.90821492927058770002e-10)));
+}
+// sin and cos of 2 pi (w + 1) / 2^32: the angle is an exact 32-bit fraction of the circle, so the quadrant and the
+// remainder theta in [-pi/4, pi/4) come from integer arithmetic; Taylor series to theta^17 / theta^18.
+__device__ __forceinline__ void fast_sincos2pi_u01(uint32_t w, double* sn, double* cs) {
+    const uint32_t kp = (w + 1u) + 0x20000000u;
+    const int q = (int)(kp >> 30), ri = (int)(kp & 0x3fffffffu) - 0x20000000;
+    const double th = (double)ri * 1.4629180792671596e-09, t2 = th * th;      // pi / 2^31
+    double S = 2.8114572543455206e-15;                              // 1 / 17!
+    S = __fma_rn(S, t2, -7.647163731819816e-13);                    // -1 / 15!
+    S = __fma_rn(S, t2, 1.6059043836821613e-10);                    // 1 / 13!
+    S = __fma_rn(S, t2, -2.505210838544172e-08);                    // -1 / 11!
+    S = __fma_rn(S, t2, 2.7557319223985893e-06);                    // 1 / 9!
+    S = __fma_rn(S, t2, -0.0001984126984126984);                    // -1 / 7!
+    S = __fma_rn(S, t2, 0.008333333333333333);                      // 1 / 5!
+    S = __fma_rn(S, t2, -0.16666666666666666);                      // -1 / 3!
+    S = __fma_rn(S * t2, th, th);
+    double Cc = -1.5619206968586225e-16;                            // -1 / 18!
+    Cc = __fma_rn(Cc, t2, 4.779477332387385e-14);                   // 1 / 16!
+    Cc = __fma_rn(Cc, t2, -1.1470745597729725e-11);                 // -1 / 14!
+    Cc = __fma_rn(Cc, t2, 2.08767569878681e-09);                    // 1 / 12!
+    Cc = __fma_rn(Cc, t2, -2.755731922398589e-07);                  // -1 / 10!
+    Cc = __fma_rn(Cc, t2, 2.48015873015873e-05);                    // 1 / 8!
+    Cc = __fma_rn(Cc, t2, -0.001388888888888889);                   // -1 / 6!
+    Cc = __fma_rn(Cc, t2, 0.041666666666666664);                    // 1 / 4!
+    Cc = __fma_rn(Cc, t2, -0.5);
+    Cc = __fma_rn(Cc, t2, 1.0);
+    const double a = (q & 1) ? Cc : S, b = (q & 1) ? S : Cc;        // sin, cos of the quadrant-rotated angle, up to sign
+    *sn = (q & 2) ? -a : a;
+    *cs = ((q + 1) & 2) ? -b : b;
+}
+// sqrt(x) for 0 <= x <~ 1e300 and 1 / sqrt(x) for x > 0 (normal range): rsqrt seed + two coupled Newton steps + one correction
+__device__ __forceinline__ double fast_sqrt64(double x) {
+    const double xs = fmax(x, 1e-300);                              // sqrt(0) -> 1e-150, below anything it is added to
+    const double y = rsqrt_approx64(xs);
+    double g = xs * y, h = 0.5 * y, r = __fma_rn(-h, g, 0.5);
+    g = __fma_rn(g, r, g); h = __fma_rn(h, r, h);
+    r = __fma_rn(-h, g, 0.5);
+    g = __fma_rn(g, r, g); h = __fma_rn(h, r, h);
+    return __fma_rn(__fma_rn(-g, g, xs), h, g);
+}
+__device__ __forceinline__ double fast_rsqrt64(double x) {
+    const double y = rsqrt_approx64(x);
+    double g = x * y, h = 0.5 * y, r = __fma_rn(-h, g, 0.5);
+    g = __fma_rn(g, r, g); h = __fma_rn(h, r, h);
+    r = __fma_rn(-h, g, 0.5);
+    h = __fma_rn(h, r, h);
+    return 2.0 * h;
+}
+
 template <class T> struct Fn;
 template <> struct Fn<float> {
     static __device__ __forceinline__ float log(float x) { return logf(x); }
@@ -452,6 +544,12 @@ template <> struct Fn<float> {
     // cos / sincos of 2 pi u for u in (0,1]: the pi-scaled forms need no range reduction of an irrational multiple
     static __device__ __forceinline__ float cos2pi(float u) { return cospif(2.0f * u); }
     static __device__ __forceinline__ void sincos2pi(float u, float* s, float* c) { sincospif(2.0f * u, s, c); }
+    // of the uniform of a Philox word (uniform01<float>): ln u, cos 2 pi u, sincos 2 pi u
+    static __device__ __forceinline__ float log_w(uint32_t w) { return logf(((float)(w >> 8) + 1.0f) * (1.0f / 16777216.0f)); }
+    static __device__ __forceinline__ float cos2pi_w(uint32_t w) { return cospif(2.0f * (((float)(w >> 8) + 1.0f) * (1.0f / 16777216.0f))); }
+    static __device__ __forceinline__ void sincos2pi_w(uint32_t w, float* s, float* c) { sincospif(2.0f * (((float)(w >> 8) + 1.0f) * (1.0f / 16777216.0f)), s, c); }
+    static __device__ __forceinline__ float sqrt01(float x) { return sqrtf(x); }
+    static __device__ __forceinline__ float rsqrt_pos(float x) { return rsqrtf(x); }
     static __device__ __forceinline__ float max0(float x) { return fmaxf(x, 0.0f); }
     static __device__ __forceinline__ bool finite(float x) { return isfinite(x); }
 };
@@ -463,6 +561,19 @@ template <> struct Fn<double> {
     static __device__ __forceinline__ void sincos(double x, double* s, double* c) { ::sincos(x, s, c); }
     static __device__ __forceinline__ double cos2pi(double u) { return ::cospi(2.0 * u); }
     static __device__ __forceinline__ void sincos2pi(double u, double* s, double* c) { ::sincospi(2.0 * u, s, c); }
+#if SUG_FAST_MATH64
+    static __device__ __forceinline__ double log_w(uint32_t w) { return fast_log_u01(w); }
+    static __device__ __forceinline__ double cos2pi_w(uint32_t w) { double s, c; fast_sincos2pi_u01(w, &s, &c); return c; }
+    static __device__ __forceinline__ void sincos2pi_w(uint32_t w, double* s, double* c) { fast_sincos2pi_u01(w, s, c); }
+    static __device__ __forceinline__ double sqrt01(double x) { return fast_sqrt64(x); }
+    static __device__ __forceinline__ double rsqrt_pos(double x) { return fast_rsqrt64(x); }
+#else
+    static __device__ __forceinline__ double log_w(uint32_t w) { return ::log(((double)w + 1.0) * (1.0 / 4294967296.0)); }
+    static __device__ __forceinline__ double cos2pi_w(uint32_t w) { return ::cospi(2.0 * (((double)w + 1.0) * (1.0 / 4294967296.0))); }
+    static __device__ __forceinline__ void sincos2pi_w(uint32_t w, double* s, double* c) { ::sincospi(2.0 * (((double)w + 1.0) * (1.0 / 4294967296.0)), s, c); }
+    static __device__ __forceinline__ double sqrt01(double x) { return ::sqrt(x); }
+    static __device__ __forceinline__ double rsqrt_pos(double x) { return ::rsqrt(x); }
+#endif
     static __device__ __forceinline__ double max0(double x) { return fmax(x, 0.0); }
     static __device__ __forceinline__ bool finite(double x) { return isfinite(x); }
 };
@@ -484,11 +595,11 @@ template <class T>
 __device__ __forceinline__ void kp_direction(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2_base, T n[3]) {
     uint32_t d[4];
     philox4x32_10(c0, c1, c2_kind(c2_base, RNG_DIR), 0u, k0, k1, d);
-    const T u1 = uniform01<T>(d[0]), u2 = uniform01<T>(d[1]);
+    const T u1 = uniform01<T>(d[0]);
     const T cos_t = (T)1 - (T)2 * u1;
-    const T sin_t = Fn<T>::sqrt(Fn<T>::max0((T)1 - cos_t * cos_t));
+    const T sin_t = Fn<T>::sqrt01(Fn<T>::max0((T)1 - cos_t * cos_t));
     T sp, cp;
-    Fn<T>::sincos2pi(u2, &sp, &cp);
+    Fn<T>::sincos2pi_w(d[1], &sp, &cp);
     n[0] = sin_t * cp; n[1] = sin_t * sp; n[2] = cos_t;
 }
 
@@ -502,9 +613,9 @@ template <class T>
 __device__ __forceinline__ void kp_attempt0(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2_base, T& Q, T& R) {
     uint32_t w[4];
     philox4x32_10(c0, c1, c2_kind(c2_base, RNG_KP), 0u, k0, k1, w);
-    const T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]), r4 = uniform01<T>(w[3]);
-    const T c = Fn<T>::cos2pi(r2);
-    Q = Fn<T>::log(r1) + c * c * Fn<T>::log(r3);
+    const T r4 = uniform01<T>(w[3]);
+    const T c = Fn<T>::cos2pi_w(w[1]);
+    Q = Fn<T>::log_w(w[0]) + c * c * Fn<T>::log_w(w[2]);
     R = r4 * r4;
 }
 
@@ -543,23 +654,22 @@ __device__ __forceinline__ int kp_draw(unsigned draw_mask, T alpha, T m_inv2a, u
             if (M > band) { used = n + 1; break; }
             if (M < -band) continue;
         }
-        T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]), r4 = uniform01<T>(w[3]);
-        T c = Fn<T>::cos2pi(r2);
-        T lambda2 = (Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) * m_inv2a;
+        T r4 = uniform01<T>(w[3]);
+        T c = Fn<T>::cos2pi_w(w[1]);
+        T lambda2 = (Fn<T>::log_w(w[0]) + c * c * Fn<T>::log_w(w[2])) * m_inv2a;
         if (r4 * r4 <= (T)1 - lambda2) { a0 = (T)1 - (T)2 * lambda2; used = n + 1; break; }
     }
     __syncwarp(converged);
     if (!used) return 0;
     if (PRETEST && !from_pre) {
-        T r1 = uniform01<T>(w[0]), r2 = uniform01<T>(w[1]), r3 = uniform01<T>(w[2]);
-        T c = Fn<T>::cos2pi(r2);
-        T lambda2 = (Fn<T>::log(r1) + c * c * Fn<T>::log(r3)) * m_inv2a;
+        T c = Fn<T>::cos2pi_w(w[1]);
+        T lambda2 = (Fn<T>::log_w(w[0]) + c * c * Fn<T>::log_w(w[2])) * m_inv2a;
         a0 = (T)1 - (T)2 * lambda2;
     }
     T n[3];
     if (dir) { n[0] = dir[0]; n[1] = dir[dir_stride]; n[2] = dir[2 * dir_stride]; }
     else kp_direction<T>(k0, k1, c0, c1, c2_base, n);
-    const T rho = Fn<T>::sqrt(Fn<T>::max0((T)1 - a0 * a0));
+    const T rho = Fn<T>::sqrt01(Fn<T>::max0((T)1 - a0 * a0));
     v[0] = a0; v[1] = rho * n[0]; v[2] = rho * n[1]; v[3] = rho * n[2];
     return used;
 }
@@ -615,7 +725,7 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
             const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
             if (ok) {
                 if (KIND == KIND_HB) {
-                    const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;          // 1/k and k without a division
+                    const T ik = Fn<T>::rsqrt_pos(n2), k = n2 * ik;      // 1/k and k without a division
                     T ud[4] = {r0 * ik, -r1 * ik, -r2 * ik, -r3 * ik};
                     T v[4];
                     used = kp_draw<T>(draw_mask, two_beta_over_nc * k, m_nc_over_4beta * ik, k0, k1, c0, c1,

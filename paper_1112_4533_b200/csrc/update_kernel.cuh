@@ -119,9 +119,16 @@ __device__ __forceinline__ void site_from_coords(const Geom& g, unsigned xh, uns
 #endif
 }
 
+// Block tiles (Geom::Bz, Bt; su_set_option "block_tile_z" / "block_tile_t") are compiled in only with -DSUG_BLOCK_TILES=1:
+// the second decode path alone made ptxas keep 544 bytes of the SU(4) fp64 kernel's matrices in local memory (OR sub-step
+// 0.093 -> 0.162 ms at 24^4), and the tiles bought nothing (profiles/r02g section 7).
+#ifndef SUG_BLOCK_TILES
+#define SUG_BLOCK_TILES 0
+#endif
 // traversal index (over the OWNED sites of one parity) -> (x/2, y, z, interior t); all indices stay in registers
 __device__ __forceinline__ void traversal_coords(const Geom& g, unsigned tix, unsigned& xh, unsigned& y, unsigned& z, unsigned& ti) {
     const unsigned row = (unsigned)g.Lxh, pl = row * (unsigned)g.L[1];
+#if SUG_BLOCK_TILES
     if (g.Bz * g.Bt > 1) {
         // block tiles: (z-chunk, t-block, z-block, x-y segment group | warp: segment, t in block, z in block | lane)
         const unsigned wb = (unsigned)g.Wb, bz = (unsigned)g.Bz, bt = (unsigned)g.Bt, sw = wb / (bz * bt);
@@ -139,6 +146,7 @@ __device__ __forceinline__ void traversal_coords(const Geom& g, unsigned tix, un
         ti = tb * bt + dt;
         return;
     }
+#endif
     const unsigned grp = pl * (unsigned)g.Zc, span = grp * (unsigned)g.Lt_int;
     const unsigned zc = tix / span;  unsigned r = tix - zc * span;
     ti = r / grp;                    r -= ti * grp;
@@ -239,9 +247,9 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
     const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
     typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
     constexpr bool STREAM_SELF = !FUSED || SUG_FUSED_STREAM;
-    if (FUSE3 == 3) {
+    if constexpr (FUSE3 == 3) {
         // two-row storage with lazy third rows (Su3Rows): three links up front per term, as FUSE3 == 1
-        static_assert(FUSE3 != 3 || (STORE == STORE_RECON12 && NC == 3 && UNR), "FUSE3 == 3 is the SU(3) two-row form");
+        static_assert(STORE == STORE_RECON12 && NC == 3 && UNR, "FUSE3 == 3 is the SU(3) two-row form");
 #pragma unroll(KUNR ? 3 : 1)
         for (int k = 0; k < 3; ++k) {
             const int nu = k + (k >= mu ? 1 : 0);
@@ -266,7 +274,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
             pre_slot(2 * k + 1);
             Su3Rows<T>::acc_lower(S, A, B, P);
         }
-    } else if (FUSE3 == 2) {
+    } else if constexpr (FUSE3 == 2) {
         // Software pipeline over the six staple terms (few warps per SM: nothing else hides the load latency). A term is
         // P = A B (or A^dagger B), then S += P C^dagger (or P C). While P is formed the term's third link C is in
         // flight; while S is accumulated the first two links of the NEXT term are (the own link after the last
@@ -569,7 +577,7 @@ __device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p
     const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
     if (ok) {
         if (KIND == KIND_HB) {
-            const T ik = Fn<T>::rsqrt(n2), k = n2 * ik;
+            const T ik = Fn<T>::rsqrt_pos(n2), k = n2 * ik;
             T ud[4] = {W[0] * ik, -W[1] * ik, -W[2] * ik, -W[3] * ik};
             T v[4];
             used = kp_draw<T>(draw_mask, (T)a.beta * k, (T)-0.5 / (T)a.beta * ik, a.k0, a.k1, s.lex, sweep_ctr,

@@ -538,8 +538,14 @@ def test_traversal_and_prefetch_knobs_are_bitwise_neutral(mods, v, dims):
         return G.export_links(), G.counters()
 
     ref = run({})
-    for opts in ({"block_tile_z": 2, "block_tile_t": 2}, {"block_tile_z": 4}, {"block_tile_t": 2}, {"block_tile_z": 2, "z_chunk_planes": 2},
-                 {"prefetch_slices": 1}, {"prefetch_slices": 3, "block_tile_z": 2}, {"blocks_per_sm": 2}):
+    probe = su.Lattice(Nc, dims, precision, recon12, kernel)
+    tiles = probe.get_option("block_tiles_supported") == 1       # compiled in only with -DSUG_BLOCK_TILES=1 (ablation builds)
+    if not tiles:
+        with pytest.raises(su.SuError):
+            probe.set_option("block_tile_z", 2)
+    tile_opts = ({"block_tile_z": 2, "block_tile_t": 2}, {"block_tile_z": 4}, {"block_tile_t": 2}, {"block_tile_z": 2, "z_chunk_planes": 2},
+                 {"prefetch_slices": 3, "block_tile_z": 2}) if tiles else ()
+    for opts in tile_opts + ({"prefetch_slices": 1}, {"prefetch_slices": 3}, {"blocks_per_sm": 2}, {"block_tile_z": 1}):
         got = run(opts)
         assert np.array_equal(got[0], ref[0]), opts
         assert got[1] == ref[1], opts
@@ -605,3 +611,28 @@ def test_cooperative_launch_falls_back_when_the_lattice_does_not_fit(mods):
     G.sweep(6.0, 1, 1)
     assert G.launch_count() - n0 == 16
     assert abs(G.plaquette() - 1.0) > 1e-3
+
+
+def test_fast_math_against_host(mods):
+    """The branch-free fp64 ln / sincos / sqrt / rsqrt of the Kennedy-Pendleton draw (csrc/su_device.cuh) against numpy in
+    long double, on 2^22 random Philox-like words plus every edge word: ln to 3e-16 relative, sin / cos to 3e-16 absolute,
+    square roots to 3e-16 relative (sqrt(0) may come out as 1e-150)."""
+    su, _ = mods
+    rng = np.random.default_rng(5)
+    edge = np.array([0, 1, 2, 3, 2**32 - 1, 2**32 - 2, 2**31, 2**31 - 1, 2**31 + 1, 2**30, 2**30 - 1, 3 * 2**30, 3 * 2**30 - 1,
+                     2**29, 2**29 - 1, 2**29 + 1, 0x6a09e667, 0xb504f333, 0xb504f334], dtype=np.uint64)
+    w = np.concatenate([rng.integers(0, 2**32, 1 << 22, dtype=np.uint64), edge]).astype(np.uint32)
+    got = su.debug_kp_math(w)
+    n = w.astype(np.longdouble) + 1
+    u = n / np.longdouble(2**32)
+    ref_log = np.log(u)
+    rel = np.abs((got[:, 0] - ref_log) / np.where(ref_log == 0, 1, ref_log)).astype(np.float64)
+    assert rel.max() < 3e-16, (rel.max(), w[rel.argmax()])
+    assert got[w == 2**32 - 1, 0].max() == 0.0                       # ln 1
+    pi = np.longdouble("3.14159265358979323846264338327950288")
+    ang = 2 * pi * (n % np.longdouble(2**32)) / np.longdouble(2**32)
+    assert np.abs(got[:, 1] - np.sin(ang)).max() < 3e-16
+    assert np.abs(got[:, 2] - np.cos(ang)).max() < 3e-16
+    assert (np.abs(got[:, 3] - np.sqrt(u)) / np.sqrt(u)).max() < 3e-16
+    x = 100 * u + np.longdouble(1e-3)
+    assert (np.abs(got[:, 4] * np.sqrt(x) - 1)).max() < 4e-16
