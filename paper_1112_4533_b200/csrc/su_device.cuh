@@ -525,6 +525,13 @@ __device__ __forceinline__ double fast_sqrt64(double x) {
     g = __fma_rn(g, r, g); h = __fma_rn(h, r, h);
     return __fma_rn(__fma_rn(-g, g, xs), h, g);
 }
+// 1 / x for x > 0 in the normal range: reciprocal seed + two Newton steps (<= 1 ulp), no slow path
+__device__ __forceinline__ double fast_rcp64(double x) {
+    double r = rcp_approx64(x);
+    r = __fma_rn(r, __fma_rn(-x, r, 1.0), r);
+    r = __fma_rn(r, __fma_rn(-x, r, 1.0), r);
+    return r;
+}
 __device__ __forceinline__ double fast_rsqrt64(double x) {
     const double y = rsqrt_approx64(x);
     double g = x * y, h = 0.5 * y, r = __fma_rn(-h, g, 0.5);
@@ -550,6 +557,7 @@ template <> struct Fn<float> {
     static __device__ __forceinline__ void sincos2pi_w(uint32_t w, float* s, float* c) { sincospif(2.0f * (((float)(w >> 8) + 1.0f) * (1.0f / 16777216.0f)), s, c); }
     static __device__ __forceinline__ float sqrt01(float x) { return sqrtf(x); }
     static __device__ __forceinline__ float rsqrt_pos(float x) { return rsqrtf(x); }
+    static __device__ __forceinline__ float rcp_pos(float x) { return 1.0f / x; }
     static __device__ __forceinline__ float max0(float x) { return fmaxf(x, 0.0f); }
     static __device__ __forceinline__ bool finite(float x) { return isfinite(x); }
 };
@@ -567,12 +575,14 @@ template <> struct Fn<double> {
     static __device__ __forceinline__ void sincos2pi_w(uint32_t w, double* s, double* c) { fast_sincos2pi_u01(w, s, c); }
     static __device__ __forceinline__ double sqrt01(double x) { return fast_sqrt64(x); }
     static __device__ __forceinline__ double rsqrt_pos(double x) { return fast_rsqrt64(x); }
+    static __device__ __forceinline__ double rcp_pos(double x) { return fast_rcp64(x); }
 #else
     static __device__ __forceinline__ double log_w(uint32_t w) { return ::log(((double)w + 1.0) * (1.0 / 4294967296.0)); }
     static __device__ __forceinline__ double cos2pi_w(uint32_t w) { return ::cospi(2.0 * (((double)w + 1.0) * (1.0 / 4294967296.0))); }
     static __device__ __forceinline__ void sincos2pi_w(uint32_t w, double* s, double* c) { ::sincospi(2.0 * (((double)w + 1.0) * (1.0 / 4294967296.0)), s, c); }
     static __device__ __forceinline__ double sqrt01(double x) { return ::sqrt(x); }
     static __device__ __forceinline__ double rsqrt_pos(double x) { return ::rsqrt(x); }
+    static __device__ __forceinline__ double rcp_pos(double x) { return 1.0 / x; }
 #endif
     static __device__ __forceinline__ double max0(double x) { return fmax(x, 0.0); }
     static __device__ __forceinline__ bool finite(double x) { return isfinite(x); }
@@ -734,7 +744,7 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
                     if (used) quat_mul(v, ud, a); else ok = false;
                 } else {
                     // a = (u~^dagger)^2 = conj(r)^2 / k^2 (eq 17): no square root, one reciprocal
-                    const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
+                    const T in2 = Fn<T>::rcp_pos(n2), m2r0 = (T)-2 * r0 * in2;
                     a[0] = fma_x(r0, r0, -fma_x(r3, r3, fma_x(r2, r2, mul_x(r1, r1)))) * in2;
                     a[1] = m2r0 * r1; a[2] = m2r0 * r2; a[3] = m2r0 * r3;
                 }

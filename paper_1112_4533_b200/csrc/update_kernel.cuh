@@ -585,7 +585,7 @@ __device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p
             if (used) quat_mul(v, ud, a4); else ok = false;
         } else {
             // a = conj(W)^2 / k^2 (eq 17)
-            const T in2 = (T)1 / n2, m2w0 = (T)-2 * W[0] * in2;
+            const T in2 = Fn<T>::rcp_pos(n2), m2w0 = (T)-2 * W[0] * in2;
             a4[0] = fma_x(W[0], W[0], -fma_x(W[3], W[3], fma_x(W[2], W[2], mul_x(W[1], W[1])))) * in2;
             a4[1] = m2w0 * W[1]; a4[2] = m2w0 * W[2]; a4[3] = m2w0 * W[3];
         }

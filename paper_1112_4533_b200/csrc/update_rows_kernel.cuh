@@ -198,7 +198,7 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
                                   c2_base | (uint32_t)sub, v);
                 if (used) quat_mul(v, ud, q4); else ok = false;
             } else {
-                const T in2 = (T)1 / n2, m2r0 = (T)-2 * r0 * in2;
+                const T in2 = Fn<T>::rcp_pos(n2), m2r0 = (T)-2 * r0 * in2;
                 q4[0] = (r0 * r0 - (r1 * r1 + r2 * r2 + r3 * r3)) * in2;
                 q4[1] = m2r0 * r1; q4[2] = m2r0 * r2; q4[3] = m2r0 * r3;
             }
