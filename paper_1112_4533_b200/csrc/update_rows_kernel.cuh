@@ -27,7 +27,12 @@ namespace sug {
 
 template <int NC> struct RowsCfg {
     static constexpr int LPW = 32 / NC;                       // links per warp
-    static constexpr int STRIDE = NC * NC + 1;                // complex elements per staged matrix (+1: bank spread)
+    // Row pitch of a staged matrix in complex elements. With pitch 8 (128 B in fp64) all rows of a matrix start in the same
+    // bank and the Nc lanes of a link, which store / read one element of Nc different rows per instruction, serialise: pitch 9
+    // (SU(8) 16^4 fp64 iteration 8.71 -> 7.70 ms). For the other Nc an odd pitch was measured too and lost (SU(6): the larger
+    // matrices leave 2 instead of 3 warps per block, OR 0.160 -> 0.169 ms; SU(4): 0.216 -> 0.223 ms): profiles/r02g section 13.
+    static constexpr int PITCH = NC + (NC % 8 == 0 ? 1 : 0);
+    static constexpr int STRIDE = NC * PITCH + 1;             // complex elements per staged matrix (+1: bank spread between links)
     static constexpr int NBUF = 5;                            // upper term: B, C; lower term: A, B, C
     static constexpr size_t bytes(int w, size_t real, int nbuf) { return (size_t)w * LPW * nbuf * STRIDE * 2 * real; }
 };
@@ -49,14 +54,21 @@ template <int NC, class T> __device__ __forceinline__ cx<T> row_pick(const cx<T>
     return v;
 }
 
+// resident blocks per SM asked of the compiler: 16 warps with 4-warp blocks, else 12 warps (as many as the registers of a
+// 168-register kernel allow), whatever the number of warps the staging buffers leave per block
+template <int NC, class T> struct RowsMinBlocks {
+    static constexpr int W = RowsWarps<NC, T>::value;
+    static constexpr int value = W == 4 ? SUG_ROWS_MINB : (W == 3 ? 4 : (W == 2 ? 6 : 8));
+};
+
 template <int NC, class T, int KIND>
-__global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k_update_rows(const UpdateArgs a) {
+__global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, RowsMinBlocks<NC, T>::value) k_update_rows(const UpdateArgs a) {
     typedef RowsCfg<NC> Cfg;
     typedef LinkIO<NC, T, STORE_FULL, true> IO;
     typedef typename IO::T2 T2;
     typedef cx<T> C;
     constexpr int WARPS = RowsWarps<NC, T>::value;
-    constexpr int LPW = Cfg::LPW, STRIDE = Cfg::STRIDE;
+    constexpr int LPW = Cfg::LPW, STRIDE = Cfg::STRIDE, PT = Cfg::PITCH;
     __shared__ C stage[WARPS * LPW][Cfg::NBUF][STRIDE];
 
     const int lane = (int)(threadIdx.x & 31u), warp = (int)(threadIdx.x >> 5);
@@ -83,7 +95,7 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
     };
     auto stage_row = [&](int buf, const C* row) {
 #pragma unroll
-        for (int c = 0; c < NC; ++c) M[buf][r * NC + c] = row[c];
+        for (int c = 0; c < NC; ++c) M[buf][r * PT + c] = row[c];
     };
 
     C S[NC], A[NC], B[NC], D[NC], P[NC];
@@ -108,14 +120,14 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
         for (int j = 0; j < NC; ++j) {
             C acc = mk<T>(0, 0);
 #pragma unroll
-            for (int q = 0; q < NC; ++q) mad(acc, A[q], M[0][q * NC + j]);
+            for (int q = 0; q < NC; ++q) mad(acc, A[q], M[0][q * PT + j]);
             P[j] = acc;
         }
 #pragma unroll
         for (int j = 0; j < NC; ++j) {
             C acc = S[j];
 #pragma unroll
-            for (int q = 0; q < NC; ++q) mad_cb(acc, P[q], M[1][j * NC + q]);
+            for (int q = 0; q < NC; ++q) mad_cb(acc, P[q], M[1][j * PT + q]);
             S[j] = acc;
         }
         // lower: U_nu(x-nu)^dagger U_mu(x-nu) U_nu(x-nu+mu)
@@ -130,14 +142,14 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
         for (int j = 0; j < NC; ++j) {
             C acc = mk<T>(0, 0);
 #pragma unroll
-            for (int q = 0; q < NC; ++q) mad_ca(acc, M[2][q * NC + r], M[3][q * NC + j]);
+            for (int q = 0; q < NC; ++q) mad_ca(acc, M[2][q * PT + r], M[3][q * PT + j]);
             P[j] = acc;
         }
 #pragma unroll
         for (int j = 0; j < NC; ++j) {
             C acc = S[j];
 #pragma unroll
-            for (int q = 0; q < NC; ++q) mad(acc, P[q], M[4][q * NC + j]);
+            for (int q = 0; q < NC; ++q) mad(acc, P[q], M[4][q * PT + j]);
             S[j] = acc;
         }
     }
@@ -155,7 +167,7 @@ __global__ void __launch_bounds__(32 * RowsWarps<NC, T>::value, SUG_ROWS_MINB) k
     for (int j = 0; j < NC; ++j) {
         C acc = mk<T>(0, 0);
 #pragma unroll
-        for (int q = 0; q < NC; ++q) mad_cb(acc, U[q], M[0][j * NC + q]);
+        for (int q = 0; q < NC; ++q) mad_cb(acc, U[q], M[0][j * PT + q]);
         W[j] = acc;
     }
 
