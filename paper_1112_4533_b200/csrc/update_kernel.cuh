@@ -200,7 +200,7 @@ __device__ __forceinline__ void prefetch_slices_ahead(const void* links, const G
 template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int FUSE3, bool KUNR, int LDN, int PRE, bool FUSED>
 __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, const int mu, const SiteNbr& s, const unsigned tix,
                                             const unsigned warp_mask, const uint32_t sweep_ctr, T* dir_col,
-                                            unsigned& att_total, unsigned& exhausted) {
+                                            unsigned& att_total, unsigned& exhausted, cx<T>* s_col = nullptr) {
     typedef LinkIO<NC, T, STORE, UNR> IO;
     typedef Mat<NC, T, UNR> M;
     typedef cx<T> C;
@@ -247,7 +247,56 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
     const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
     typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
     constexpr bool STREAM_SELF = !FUSED || SUG_FUSED_STREAM;
-    if constexpr (FUSE3 == 3) {
+    if constexpr (FUSE3 == 4) {
+        // The staple sum lives in shared memory (one private column per thread, s_col[e * BLOCK]) while the six terms are
+        // formed: 36 (fp64) registers fewer during the phase that holds three loaded links, so that a 128-register budget -
+        // 16 instead of 12 warps per SM, a third more loads in flight - does not spill. Terms as in FUSE3 == 1 (three
+        // links up front, row by row); the same sums in the same order.
+        auto term = [&](bool upper, bool first) {
+#pragma unroll
+            for (int i = 0; i < NC; ++i) {
+                C r[NC];
+#pragma unroll
+                for (int j = 0; j < NC; ++j) {
+                    C acc = mk<T>(0, 0);
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) { if (upper) mad(acc, A[i * NC + k], B[k * NC + j]); else mad_ca(acc, A[k * NC + i], B[k * NC + j]); }
+                    r[j] = acc;
+                }
+#pragma unroll
+                for (int j = 0; j < NC; ++j) {
+                    C acc = first ? mk<T>(0, 0) : s_col[(i * NC + j) * BLOCK];
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) { if (upper) mad_cb(acc, r[k], P[j * NC + k]); else mad(acc, r[k], P[k * NC + j]); }
+                    s_col[(i * NC + j) * BLOCK] = acc;
+                }
+            }
+        };
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int nu = k + (k >= mu ? 1 : 0);
+            const int dpnu = sel4(nu, s.dp[0], s.dp[1], s.dp[2], s.dp[3]);
+            const int dmnu = sel4(nu, s.dm[0], s.dm[1], s.dm[2], s.dm[3]);
+            const typename IO::T2* pl_nu_s = IO::plane((const void*)a.links, a.g, nu, p);
+            const typename IO::T2* pl_nu_o = IO::plane((const void*)a.links, a.g, nu, 1 - p);
+            IO::template load<LDN>(pl_mu_o, cb + (unsigned)dpnu, B);
+            IO::template load<LDN>(pl_nu_o, cb + (unsigned)dpmu, P);
+            IO::template load<LDN>(pl_nu_s, cb, A);
+            term(true, k == 0);
+            if (LDT != LDN && nu == 3) {
+                IO::template load<LDT>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load<LDT>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load<LDT>(pl_nu_o, cb + (unsigned)dmnu, A);
+            } else {
+                IO::template load<LDN>(pl_mu_o, cb + (unsigned)dmnu, B);
+                IO::template load<LDN>(pl_nu_s, cb + (unsigned)(dmnu + dpmu), P);
+                IO::template load<LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
+            }
+            term(false, false);
+        }
+#pragma unroll
+        for (int e = 0; e < NC * NC; ++e) S[e] = s_col[e * BLOCK];
+    } else if constexpr (FUSE3 == 3) {
         // two-row storage with lazy third rows (Su3Rows): three links up front per term, as FUSE3 == 1
         static_assert(STORE == STORE_RECON12 && NC == 3 && UNR, "FUSE3 == 3 is the SU(3) two-row form");
 #pragma unroll(KUNR ? 3 : 1)
@@ -422,6 +471,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
     constexpr int PRE_ASKED = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
     constexpr int PRE = (PRE_ASKED == 4 && !FUSE3) ? (sizeof(T) == 4 ? 1 : 0) : PRE_ASKED;     // 4 needs the three-link staple terms
     __shared__ T dir_sm[PRE >= 2 ? 5 * NSUB : (PRE == 1 ? 3 * NSUB : 1)][PRE ? BLOCK : 1];
+    __shared__ cx<T> s_sm[FUSE3 == 4 ? NC * NC : 1][FUSE3 == 4 ? BLOCK : 1];      // FUSE3 == 4: the staple sums
     const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
     unsigned att_total = 0, exhausted = 0;
     if (!FUSED) {
@@ -434,7 +484,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
             if (a.pf_slices > 0)
                 prefetch_slices_ahead<LinkIO<NC, T, STORE, UNR>::E, typename V2<T>::type>(a.links, a.g, __shfl_sync(warp_mask, s.cb, 0), a.pf_slices);
             update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, SUG_NEIGHBOUR_LD, PRE, false>(
-                a, a.parity, a.mu, s, tix, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
+                a, a.parity, a.mu, s, tix, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted,
+                &s_sm[0][FUSE3 == 4 ? threadIdx.x : 0]);
         }
     } else {
         __shared__ unsigned sh_ticket, sh_epoch, sh_ready[2];     // sh_ready alternates per phase: no reuse race
@@ -476,7 +527,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
                 if (a.pf_slices > 0 && st == 0)             // the first stage is the one that touches links for the first time
                     prefetch_slices_ahead<LinkIO<NC, T, STORE, UNR>::E, typename V2<T>::type>(a.links, a.g, __shfl_sync(warp_mask, s.cb, 0), a.pf_slices);
                 update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, SUG_FUSED_LD, PRE, true>(
-                    a, p, mu, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
+                    a, p, mu, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted,
+                    &s_sm[0][FUSE3 == 4 ? threadIdx.x : 0]);
             }
             int nx = st + 1;
             while (nx < g && __ldg(work + nx) == FUSED_NONE) ++nx;
@@ -661,6 +713,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_coop(const UpdateArgs a)
     constexpr int PRE_ASKED = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
     constexpr int PRE = (PRE_ASKED == 4 && !FUSE3) ? (sizeof(T) == 4 ? 1 : 0) : PRE_ASKED;
     __shared__ T dir_sm[PRE >= 2 ? 5 * NSUB : (PRE == 1 ? 3 * NSUB : 1)][PRE ? BLOCK : 1];
+    __shared__ cx<T> s_sm[FUSE3 == 4 ? NC * NC : 1][FUSE3 == 4 ? BLOCK : 1];
     const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
     const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = tix < a.g.Vh_int;
@@ -677,7 +730,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_coop(const UpdateArgs a)
                 SiteNbr s;
                 site_of_thread(a.g, tix, sub >> 2, s);
                 update_link<NC, T, STORE, KIND, UNR, BLOCK, FUSE3, KUNR, LD_CG, PRE, true>(
-                    b, sub >> 2, sub & 3, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted);
+                    b, sub >> 2, sub & 3, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted,
+                    &s_sm[0][FUSE3 == 4 ? threadIdx.x : 0]);
             }
             grid.sync();
         }
