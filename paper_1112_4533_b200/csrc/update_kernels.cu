@@ -132,8 +132,20 @@ template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB> static 
 #ifndef SUG_CFG_SU3R_F32_OR
 #define SUG_CFG_SU3R_F32_OR Cfg<128, SUG_SU3R_F32_MINB, SUG_SU3R_SMODE, true>
 #endif
+#ifndef SUG_SU4_F64_HB_BLOCK
+#define SUG_SU4_F64_HB_BLOCK 128
+#endif
+#ifndef SUG_SU4_F64_HB_MINB
+#define SUG_SU4_F64_HB_MINB 1
+#endif
+#ifndef SUG_SU4_F64_HB_SMODE
+#define SUG_SU4_F64_HB_SMODE 0
+#endif
+#ifndef SUG_SU4_F64_HB_KUNR
+#define SUG_SU4_F64_HB_KUNR false
+#endif
 #ifndef SUG_CFG_SU4_F64_HB
-#define SUG_CFG_SU4_F64_HB Cfg<128, 1>
+#define SUG_CFG_SU4_F64_HB Cfg<SUG_SU4_F64_HB_BLOCK, SUG_SU4_F64_HB_MINB, SUG_SU4_F64_HB_SMODE, SUG_SU4_F64_HB_KUNR>
 #endif
 #ifndef SUG_CFG_SU4_F64_OR
 #define SUG_CFG_SU4_F64_OR Cfg<128, 2, true, true>
