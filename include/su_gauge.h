@@ -193,7 +193,9 @@ su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* o
  *                     passes in another, with grid barriers where the launch boundaries were (register kernels of
  *                     Nc <= 4, lattices whose V/2 threads are resident at once, not slabs; otherwise plain launches;
  *                     su_get_option "coop_sweep_effective": bit 0 heatbath, bit 1 overrelaxation). Bitwise the plain
- *                     sweep (tested). Measured no faster than the CUDA-graph replay of the 40 launches (profiles/r02g).
+ *                     sweep (tested). With at most 16 blocks per sub-step (8^4) the grid is one thread-block cluster and the
+ *                     barrier the hardware cluster barrier. Measured 0 - 13 % faster than the CUDA-graph replay of the 40
+ *                     launches at 8^4, no faster at 16^4 (profiles/r02g).
  *   "block_tile_z", "block_tile_t"   the warps of a thread block of the Nc = 3, 4 register kernels work on the same x-y
  *                     segments of this many consecutive z-planes / time slices (1: a block is consecutive segments of
  *                     one plane), dropped silently where the lattice or the block does not divide evenly. Only in libraries built

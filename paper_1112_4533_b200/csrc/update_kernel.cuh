@@ -60,6 +60,7 @@ struct UpdateArgs {
     int pf_slices;                     // > 0: every warp asks L2 for the link tiles of its sites' positions this many time slices ahead
     int dyn_smem;                      // host side only: unused dynamic shared memory per block (caps the resident blocks per SM)
     int coop_passes;                   // > 0: cooperative launch that runs this many whole passes (8 sub-steps each) with grid barriers
+    int coop_cluster;                  // set by the launcher: the whole grid is ONE thread-block cluster (<= 16 blocks): cluster barriers
     uint8_t* attempts;                 // device, [n_sub][Vh] or NULL
     unsigned long long* counters;      // device, {kp_attempts_total, kp_exhausted}
     // slab mode: link buffers of the slabs below / above in t (peer memory over NVLink, or this device). The
@@ -704,11 +705,17 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2(const UpdateArgs a) 
 // same arithmetic as the plain launches (bitwise equal); neighbour links are read with ld.global.cg (L2 only), which
 // needs no L1 invalidation to see what other blocks stored before the barrier. a.pass = number of the first pass;
 // a.reunit applies to the last pass of the launch. Not for slab handles (no halo push in here).
+// When the sub-step has at most 16 blocks (SU(2) / SU(3) 8^4: 2048 sites of one parity = 16 x 128 threads) the launcher makes
+// the whole grid one thread-block cluster and the barrier is the hardware cluster barrier (barrier.cluster, release /
+// acquire at cluster scope, ~0.2 us) instead of the cooperative-groups grid barrier (atomics through L2, ~2 us).
+__device__ __forceinline__ void coop_barrier(const UpdateArgs& a) {
+    namespace cg = cooperative_groups;
+    if (a.coop_cluster) cg::this_cluster().sync();
+    else cg::this_grid().sync();
+}
 // ------------------------------------------------------------------------------------------
 template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, int FUSE3 = 0, bool KUNR = false>
 __global__ void __launch_bounds__(BLOCK, MINB) k_update_coop(const UpdateArgs a) {
-    namespace cg = cooperative_groups;
-    cg::grid_group grid = cg::this_grid();
     constexpr int NSUB = NC * (NC - 1) / 2;
     constexpr int PRE_ASKED = ((KIND == KIND_HB) && UNR) ? (sizeof(T) == 4 ? SUG_KP_PRE_F32 : SUG_KP_PRE_F64) : 0;
     constexpr int PRE = (PRE_ASKED == 4 && !FUSE3) ? (sizeof(T) == 4 ? 1 : 0) : PRE_ASKED;
@@ -733,7 +740,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_coop(const UpdateArgs a)
                     b, sub >> 2, sub & 3, s, 0u, warp_mask, sweep_ctr, &dir_sm[0][PRE ? threadIdx.x : 0], att_total, exhausted,
                     &s_sm[0][FUSE3 == 4 ? threadIdx.x : 0]);
             }
-            grid.sync();
+            coop_barrier(a);
         }
     }
     if (KIND == KIND_HB) flush_kp_counters(a, att_total, exhausted);
@@ -741,8 +748,6 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_coop(const UpdateArgs a)
 
 template <class T, int KIND, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2_coop(const UpdateArgs a) {
-    namespace cg = cooperative_groups;
-    cg::grid_group grid = cg::this_grid();
     const uint32_t sweep_ctr = a.sweep_ptr ? *a.sweep_ptr : a.sweep;
     const unsigned tix = blockIdx.x * BLOCK + threadIdx.x;
     const bool active = tix < a.g.Vh_int;
@@ -760,7 +765,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update_su2_coop(const UpdateArg
                 site_of_thread(a.g, tix, sub >> 2, s);
                 update_link_su2<T, KIND, LD_CG, false>(b, sub >> 2, sub & 3, s, tix, warp_mask, sweep_ctr, att_total, exhausted);
             }
-            grid.sync();
+            coop_barrier(a);
         }
     }
     if (KIND == KIND_HB) flush_kp_counters(a, att_total, exhausted);

@@ -40,7 +40,33 @@ template <class K> static void launch_k(K kern, unsigned grid, int block, cudaSt
 }
 
 // cooperative whole-pass launch (k_update_coop): every block of a sub-step resident at once, grid barriers inside
-template <class K> static cudaError_t launch_coop(K kern, unsigned grid, int block, cudaStream_t st, const UpdateArgs& a) {
+template <class K> static cudaError_t launch_coop(K kern, unsigned grid, int block, cudaStream_t st, const UpdateArgs& a0) {
+    UpdateArgs a = a0;
+    if (grid <= 16) {
+        // the whole sub-step is at most 16 blocks: one thread-block cluster, hardware cluster barriers between the sub-steps
+        static std::mutex mu;
+        static std::map<const void*, int> state;          // 0 unknown, 1 cluster launches work for this kernel, -1 they do not
+        int st_k;
+        { std::lock_guard<std::mutex> lock(mu); st_k = state[(const void*)kern]; }
+        if (st_k == 0) {
+            st_k = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess ? 1 : -1;
+            cudaGetLastError();
+        }
+        if (st_k == 1) {
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = grid; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            a.coop_cluster = 1;
+            const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, a);
+            { std::lock_guard<std::mutex> lock(mu); state[(const void*)kern] = e == cudaSuccess ? 1 : -1; }
+            if (e == cudaSuccess) return e;
+            cudaGetLastError();                           // e.g. the cluster does not fit: fall back to the grid barrier
+        }
+    }
+    a.coop_cluster = 0;
     void* args[] = {(void*)&a};
     return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(block), args, 0, st);
 }
