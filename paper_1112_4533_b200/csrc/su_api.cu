@@ -31,6 +31,7 @@ struct su_lattice {
     size_t link_bytes = 0;         // bytes of one stored link
     double* d_partials = nullptr;
     double* d_result = nullptr;
+    double* h_result = nullptr;    // pinned host copy of d_result (2 doubles): the read-back of a reduction is one async copy + sync
     unsigned long long* d_counters = nullptr;
     uint32_t* d_sweep = nullptr;
     uint8_t* d_attempts = nullptr;
@@ -538,6 +539,7 @@ static su_status create_common(int Nc, int Lx, int Ly, int Lz, int Lt_glob, bool
                                          : (size_t)plaquette_blocks(h->g.Vh) + 2 * (size_t)reduce_blocks(Vs)) + 2;
     if (st == SU_OK && cudaMalloc(&h->d_partials, npart * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_result, 2 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
+    if (st == SU_OK && cudaMallocHost(&h->h_result, 2 * sizeof(double)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_counters, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMalloc(&h->d_sweep, sizeof(uint32_t)) != cudaSuccess) st = SU_ENOMEM;
     if (st == SU_OK && cudaMemset(h->d_counters, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) st = SU_ECUDA;
@@ -640,6 +642,7 @@ su_status su_lattice_destroy(su_lattice* h) {
     if (h->owns_links && h->links) cudaFree(h->links);
     if (h->d_partials) cudaFree(h->d_partials);
     if (h->d_result) cudaFree(h->d_result);
+    if (h->h_result) cudaFreeHost(h->h_result);
     if (h->d_counters) cudaFree(h->d_counters);
     if (h->d_sweep) cudaFree(h->d_sweep);
     if (h->d_attempts) cudaFree(h->d_attempts);
@@ -767,8 +770,9 @@ su_status su_plaquette(su_lattice* h, double* out) {
     AuxArgs a = aux_args(h);
     SU_CUDA(h, SU_BY_NC(h, plaquette_nc, h->var, a, h->stream, &h->n_launch), "plaquette kernels");
     double v = 0;
-    SU_CUDA(h, cudaMemcpyAsync(&v, h->d_result, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "plaquette copy");
+    SU_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "plaquette copy");
     SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_plaquette synchronise");
+    v = h->h_result[0];
     if (su_status fs = check_fused_error(h)) return fs;
     *out = v;
     return SU_OK;
@@ -782,8 +786,9 @@ su_status su_polyakov(su_lattice* h, double out[2]) {
     AuxArgs a = aux_args(h);
     SU_CUDA(h, SU_BY_NC(h, polyakov_nc, h->var, a, h->stream, &h->n_launch), "polyakov kernels");
     double v[2] = {0, 0};
-    SU_CUDA(h, cudaMemcpyAsync(v, h->d_result, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream), "polyakov copy");
+    SU_CUDA(h, cudaMemcpyAsync(h->h_result, h->d_result, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream), "polyakov copy");
     SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_polyakov synchronise");
+    v[0] = h->h_result[0]; v[1] = h->h_result[1];
     out[0] = v[0]; out[1] = v[1];
     return SU_OK;
 }
