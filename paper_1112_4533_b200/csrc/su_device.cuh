@@ -336,6 +336,22 @@ template <int NC, class T, bool UNR> struct Mat {
             }
         }
     }
+    // B <- A^dagger B in place, column by column (column j of the product needs column j of B only); same sums as mul_dn
+    static __device__ __forceinline__ void mul_dn_inplace(const C* A, C* B) {
+#pragma unroll(UNR ? NC : 1)
+        for (int j = 0; j < NC; ++j) {
+            C col[NC];
+#pragma unroll(UNR ? NC : 1)
+            for (int i = 0; i < NC; ++i) {
+                C s = mk<T>(0, 0);
+#pragma unroll(UNR ? NC : 1)
+                for (int k = 0; k < NC; ++k) mad_ca(s, A[k * NC + i], B[k * NC + j]);
+                col[i] = s;
+            }
+#pragma unroll(UNR ? NC : 1)
+            for (int i = 0; i < NC; ++i) B[i * NC + j] = col[i];
+        }
+    }
     // Re Tr (A B^dagger) = sum_ij Re(A_ij conj(B_ij))
     static __device__ __forceinline__ T retr_nd(const C* A, const C* B) {
         T s = 0;

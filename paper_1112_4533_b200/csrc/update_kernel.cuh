@@ -18,6 +18,10 @@
 
 namespace sug {
 
+// three-links-up-front staple: request the own link before the last accumulation (see update_link)
+#ifndef SUG_EARLY_SELF
+#define SUG_EARLY_SELF 0
+#endif
 #ifndef SUG_TMINUS_STREAM
 #define SUG_TMINUS_STREAM 1
 #endif
@@ -245,6 +249,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
 
     C S[NC * NC], A[NC * NC], B[NC * NC], P[NC * NC];
     M::zero(S);
+    bool self_loaded = false;
     const typename IO::T2* pl_mu_o = IO::plane((const void*)a.links, a.g, mu, 1 - p);
     typename IO::T2* pl_self = IO::plane(a.links, a.g, mu, p);
     constexpr bool STREAM_SELF = !FUSED || SUG_FUSED_STREAM;
@@ -390,7 +395,16 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
                 IO::template load<LDN>(pl_nu_o, cb + (unsigned)dmnu, A);
             }
             pre_slot(2 * k + 1);
-            M::acc_dnn(S, A, B, P);
+            if (SUG_EARLY_SELF && UNR && k == 2) {
+                // last term in two steps, B <- A^dagger B in place: A is free before the accumulation, so the own link (the
+                // eighth and last load wait of the site) is requested now and arrives while S += B P runs. Same sums.
+                M::mul_dn_inplace(A, B);
+                IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, A);
+                M::acc_nn(S, B, P);
+                self_loaded = true;
+            } else {
+                M::acc_dnn(S, A, B, P);
+            }
         } else {
             // upper: U_nu(x) U_mu(x+nu) U_nu(x+mu)^dagger
             IO::template load<LDN>(pl_nu_s, cb, A);
@@ -409,7 +423,7 @@ __device__ __forceinline__ void update_link(const UpdateArgs& a, const int p, co
     }
     C* U = A;
     C* W = B;
-    if (FUSE3 != 2) IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, U);
+    if (FUSE3 != 2 && !self_loaded) IO::template load<STREAM_SELF ? LD_STREAM : LDN>(pl_self, cb, U);
     M::mul_nd(U, S, W);                                   // W = U S^dagger
     update_subgroups<NC, T, KIND, UNR>(U, W, (T)a.beta, a.k0, a.k1, s.lex, sweep_ctr,
                                        pack_c2((int)a.pass, p, mu, 0),
