@@ -303,7 +303,8 @@ bool reunit_in_kernel(const su_lattice* h) { return !h->var.generic && h->Nc <= 
 int occupancy_cap_bytes(const su_lattice* h) {
     if (h->blocks_per_sm <= 0) return 0;
     const int per_sm = 227 * 1024, reserve = 1024 + 8 * 1024;     // 1 KB per block is the system's; headroom for static shared memory
-    return per_sm / h->blocks_per_sm - reserve;
+    const int bytes = per_sm / h->blocks_per_sm - reserve;
+    return bytes > 0 ? bytes : 0;                                  // more blocks than shared memory could ever limit: no cap
 }
 
 // Block tiles (Geom::Bz, Bt, Wb) for the launch of one sub-step, if the register kernel of this variant and kind can
