@@ -127,11 +127,23 @@ template <int NC, class T, int STORE, bool UNR, class HB, class OR = HB> static 
 #ifndef SUG_CFG_SU3_F64_OR
 #define SUG_CFG_SU3_F64_OR Cfg<SUG_SU3_F64_BLOCK, SUG_SU3_F64_MINB, SUG_SU3_F64_SMODE, true>
 #endif
+#ifndef SUG_SU3_F32_SMODE
+#define SUG_SU3_F32_SMODE 1
+#endif
+#ifndef SUG_SU3_F32_OR_MINB
+#define SUG_SU3_F32_OR_MINB 5
+#endif
+#ifndef SUG_SU3_F32_HB_MINB
+#define SUG_SU3_F32_HB_MINB 5
+#endif
+#ifndef SUG_SU3_F32_BLOCK
+#define SUG_SU3_F32_BLOCK 128
+#endif
 #ifndef SUG_CFG_SU3_F32_HB
-#define SUG_CFG_SU3_F32_HB Cfg<128, 4, true, true>
+#define SUG_CFG_SU3_F32_HB Cfg<SUG_SU3_F32_BLOCK, SUG_SU3_F32_HB_MINB, SUG_SU3_F32_SMODE, true>
 #endif
 #ifndef SUG_CFG_SU3_F32_OR
-#define SUG_CFG_SU3_F32_OR Cfg<128, 5, true, true>
+#define SUG_CFG_SU3_F32_OR Cfg<SUG_SU3_F32_BLOCK, SUG_SU3_F32_OR_MINB, SUG_SU3_F32_SMODE, true>
 #endif
 // two-row storage: staple form (1: every link completed on load, 3: lazy third rows, Su3Rows) and register caps
 #ifndef SUG_SU3R_SMODE
