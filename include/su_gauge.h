@@ -240,6 +240,40 @@ su_status su_measure_l2_peak(int device, int through_l1, double* gbs, double* ms
  * out[5 i + 0..4] = ln u, sin 2 pi u, cos 2 pi u, sqrt u, 1 / sqrt(100 u + 0.001). Host pointers; synchronises. */
 su_status su_debug_kp_math(int device, const uint32_t* words, size_t n, double* out);
 
+/* ---- a measurement that allocates nothing ----
+ * su_plaquette_static: the mean plaquette (eq 4; the quantity su_plaquette returns) of a link buffer
+ * the caller already holds, with no su_lattice handle and without a single cudaMalloc, cudaFree, cudaMallocHost or
+ * other allocating call inside the library. It is meant for the callers that cannot allocate: a job whose lattices
+ * (or whose host program's memory pool, e.g. PyTorch's caching allocator) already occupy the GPU's memory, so that a
+ * library-side cudaMalloc would fail or bypass that pool; monitoring code inside a running generation loop, where
+ * cudaMalloc / cudaFree may synchronise the device and stall the sweeps on other streams; and a process that only
+ * maps another owner's link buffer (su_ipc_open, a tensor of the host framework) and has no handle to measure with.
+ * (su_lattice_create allocates five small device buffers and one pinned host buffer; su_plaquette then uses them.)
+ *   - The only scratch the reduction needs, one partial sum per thread block, lives in a fixed 1 MiB __device__ array
+ *     inside the library image. Every GPU on which libsugauge is loaded holds that 1 MiB until the process exits.
+ *     It bounds the lattice: at most SU_STATIC_MAX_SITES = 64^4 sites; a larger lattice returns SU_EUNSUPPORTED and
+ *     launches nothing. Nc = 2, 3, 4 only (the register layouts; RECON12 for Nc = 3), else SU_EUNSUPPORTED.
+ *   - device_links: DEVICE pointer (input, read only, 16-byte aligned) to links in the library's device layout, i.e.
+ *     the buffer of su_options::buffer / su_slab_links of a whole (non-slab) lattice with the same Nc, extents,
+ *     precision and storage; links_bytes >= su_lattice_bytes(...). device_out: DEVICE pointer (output) to one double.
+ *     Both stay the caller's. device: CUDA ordinal, -1 = current. stream: cudaStream_t, NULL = legacy default stream.
+ *   - Asynchronous: two kernels are enqueued on `stream`; *device_out is valid once they have run. Nothing is copied
+ *     to the host and the call does not synchronise.
+ *   - The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, which may load the
+ *     library's device code there); make that first call during set-up, before any stream capture and outside
+ *     time-critical code. Later calls on that device only launch.
+ *   - All calls on a device share the one array, and it keeps what the last call left. Each call overwrites every
+ *     slot it later reads, so nothing has to start at zero and nothing is cleared. Two calls whose kernels can overlap
+ *     on the GPU (different streams, several host threads, several lattices) race on it and give garbage: order them.
+ *   - Under the default traversal rule the value is bit for bit su_plaquette's of the same links.
+ * Errors: SU_EINVAL (null / misaligned pointers, bad extents, precision, storage, links_bytes too small),
+ * SU_EUNSUPPORTED (too many sites, Nc > 4, device ordinal >= 64), SU_ECUDA. su_static_last_error() returns the text of
+ * the calling thread's last failure in su_plaquette_static ("" after a success); owned by the library. */
+#define SU_STATIC_MAX_SITES 16777216LL
+su_status su_plaquette_static(int Nc, int Lx, int Ly, int Lz, int Lt, su_precision p, su_storage s, int device,
+                              void* stream, const void* device_links, size_t links_bytes, double* device_out);
+const char* su_static_last_error(void);
+
 /* Text of the last error on this handle ("" if none); static text if the handle is NULL.
  * Owned by the library, valid until the next call on the handle. */
 const char* su_last_error(const su_lattice*);

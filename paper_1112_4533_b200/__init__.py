@@ -33,6 +33,7 @@ ABI_SYMBOLS = (
     "su_lattice_create_slab", "su_slab_bytes", "su_slab_links", "su_slab_set_peers", "su_slab_halo_push",
     "su_ipc_export", "su_ipc_open", "su_ipc_close", "su_slab_plaquette_sum", "su_set_option", "su_get_option",
     "su_measure_fma_peak", "su_measure_l2_peak", "su_debug_kp_math", "su_save_config", "su_load_config", "su_fused_schedule_debug", "su_fused_dep_debug",
+    "su_plaquette_static", "su_static_last_error",
 )
 
 
@@ -105,6 +106,9 @@ def lib():
     for name in ABI_SYMBOLS:
         if name not in ("su_lattice_bytes", "su_slab_bytes", "su_last_error"):
             getattr(L, name).restype = I
+    L.su_plaquette_static.argtypes = [I] * 8 + [P, P, C.c_size_t, P]
+    L.su_static_last_error.argtypes = []
+    L.su_static_last_error.restype = C.c_char_p
     _lib = L
     return L
 
@@ -148,6 +152,23 @@ def measure_l2_peak(device=-1, through_l1=False):
     if st != SU_OK:
         raise SuError(st, "su_measure_l2_peak")
     return g.value, ms.value, bpc.value
+
+
+SU_STATIC_MAX_SITES = 64 ** 4
+
+
+def plaquette_static(Nc, dims, precision, recon12, links_ptr, links_bytes, out_ptr, stream_ptr=None, device=-1):
+    """su_plaquette_static: enqueue the mean plaquette of the DEVICE link buffer `links_ptr` (library layout, whole
+    lattice) into the DEVICE double at `out_ptr`, on the cudaStream_t `stream_ptr`. For callers that must not
+    allocate GPU memory (their pool owns it all, or they sit in a running loop where cudaMalloc would stall the
+    device): the library allocates nothing here; its partial sums go to a fixed 1 MiB array inside the library, which
+    limits the lattice to SU_STATIC_MAX_SITES = 64^4 sites and is shared by every call on the device, so calls that
+    could overlap on the GPU must be ordered by the caller. Asynchronous; raises SuError with the library's text."""
+    st = lib().su_plaquette_static(int(Nc), *[int(d) for d in dims], _prec(precision),
+                                   SU_STORE_RECON12 if recon12 else SU_STORE_FULL, int(device),
+                                   C.c_void_p(stream_ptr), C.c_void_p(links_ptr), int(links_bytes), C.c_void_p(out_ptr))
+    if st != SU_OK:
+        raise SuError(st, "su_plaquette_static", (lib().su_static_last_error() or b"").decode())
 
 
 class Lattice:

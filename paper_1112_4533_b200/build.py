@@ -26,7 +26,7 @@ HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", "update_rows_k
 
 
 def _units():
-    units = [("su_api.cu", None), ("fused_schedule.cu", None), ("big_kernels.cu", None)]
+    units = [("su_api.cu", None), ("fused_schedule.cu", None), ("big_kernels.cu", None), ("static_scratch.cu", None)]
     for nc in NCS:
         units.append(("update_kernels.cu", nc))
         units.append(("aux_kernels.cu", nc))
