@@ -146,9 +146,12 @@ class DistributedLattice:
 
     def _order(self):
         if self.order == "nccl":
-            # stream-ordered: the collective waits for the kernels already enqueued on the current stream
-            # (the lattice's stream) and later kernels on that stream wait for it
-            self.dist.all_reduce(self._token)
+            # stream-ordered: the collective waits for the kernels already enqueued on the lattice's stream and later
+            # kernels on that stream wait for it. NCCL enqueues on torch's CURRENT stream, which need not be the one
+            # the Lattice captured at construction (a caller inside `with torch.cuda.stream(...)`): select it here,
+            # or the all-reduce would order nothing and the peer halo stores would race
+            with self.torch.cuda.stream(self.lat.stream):
+                self.dist.all_reduce(self._token)
         else:
             self.lat.synchronize()
             self.dist.barrier()

@@ -16,11 +16,20 @@ def main():
     import torch.distributed as dist
     from paper_1112_4533_b200.slab import DistributedLattice
 
-    torch.cuda.set_device(0)
-    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    # "shared" (default): every rank on cuda:0, gloo, host ordering. "multi": rank r on cuda:r, NCCL, the stream-ordered
+    # all-reduce between sub-steps and peer stores that really cross NVLink (needs >= world GPUs)
+    multi = len(sys.argv) > 5 and sys.argv[5] == "multi"
+    dev = rank if multi else 0
+    torch.cuda.set_device(dev)
+    if multi:
+        dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world,
+                                device_id=torch.device("cuda", dev))
+    else:
+        dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
     cfg = np.load(os.path.join(tmp, "cfg.npy"), allow_pickle=True).item()
     start = np.load(os.path.join(tmp, "start.npy"))
-    D = DistributedLattice(cfg["Nc"], cfg["dims"], cfg["precision"], cfg["recon12"], cfg["kernel"], device=0, order="host")
+    D = DistributedLattice(cfg["Nc"], cfg["dims"], cfg["precision"], cfg["recon12"], cfg["kernel"], device=dev,
+                           order="nccl" if multi else "host")
     lt = cfg["dims"][3] // world
     D.import_links(start[rank * lt:(rank + 1) * lt])
     D.sweep_counter, D.seed = cfg["sweep0"], cfg["seed"]

@@ -72,6 +72,20 @@ def test_world_size_one_over_nccl_is_the_plain_lattice(mods):
     (3, "fp64", False, "auto", 6.0), (3, "fp32", True, "auto", 6.0), (2, "fp64", False, "auto", 2.3),
     (4, "fp64", False, "generic", 11.0)], ids=["su3-fp64", "su3-fp32-r12", "su2-fp64", "su4-generic"])
 def test_two_processes_one_gpu_ipc_and_peer_halo_push(mods, tmp_path, Nc, precision, recon12, kernel, beta):
+    _two_ranks_against_the_single_lattice(mods, tmp_path, Nc, precision, recon12, kernel, beta, "shared")
+
+
+def test_two_processes_two_gpus_nccl_ordering(mods, tmp_path):
+    """The real N > 1 path: rank r on cuda:r, order="nccl" (the stream-ordered all-reduce between sub-steps), peer
+    stores over NVLink. Skips on a box with one GPU - which is every box this repository has been run on so far, so
+    this test has not executed yet."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    _two_ranks_against_the_single_lattice(mods, tmp_path, 3, "fp64", False, "auto", 6.0, "multi")
+
+
+def _two_ranks_against_the_single_lattice(mods, tmp_path, Nc, precision, recon12, kernel, beta, mode):
     su, oracle = mods
     O = oracle.OracleLattice(Nc, DIMS, precision, recon12)
     O.init_hot(9)
@@ -85,7 +99,7 @@ def test_two_processes_one_gpu_ipc_and_peer_halo_push(mods, tmp_path, Nc, precis
     np.save(tmp_path / "cfg.npy", dict(Nc=Nc, dims=DIMS, precision=precision, recon12=recon12, kernel=kernel,
                                        beta=beta, seed=9, sweep0=n_therm), allow_pickle=True)
     port = str(_free_port())
-    procs = [subprocess.Popen([sys.executable, os.path.join(HERE, "dist_worker.py"), str(r), "2", port, str(tmp_path)],
+    procs = [subprocess.Popen([sys.executable, os.path.join(HERE, "dist_worker.py"), str(r), "2", port, str(tmp_path), mode],
                               stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for r in range(2)]
     outs = []
     for p in procs:
