@@ -106,7 +106,11 @@ su_status su_import_links(su_lattice*, const double* host_src, size_t n_doubles)
  * layout), and a 64-bit FNV-1a checksum of both. su_load_config needs a handle of the same Nc and extents (any
  * precision / storage), verifies the checksum and that the plaquette it measures after the import matches the
  * header, and restores the RNG seed and sweep counter: load + su_sweep continues the writer's chain exactly when
- * precision and storage agree. Host-side I/O; both synchronise. Not available on slab handles. */
+ * precision and storage agree. Host-side I/O; both synchronise. Not available on slab handles.
+ * A file that cannot be opened, is truncated, belongs to another lattice, has header fields out of range or a wrong
+ * checksum is refused (SU_EINVAL) with the handle untouched. The plaquette can only be compared after the links are on
+ * the device: a file that fails that last check has overwritten the links, and the handle is then uninitialised
+ * (SU_ESTATE until su_init_* / su_import_links / a successful load); its RNG seed and sweep counter are unchanged. */
 su_status su_save_config(su_lattice*, const char* path);
 su_status su_load_config(su_lattice*, const char* path);
 
@@ -183,6 +187,12 @@ su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* o
  *                     Ignored (plain launches) in slab mode and for kernels without a fused form; su_get_option
  *                     "fuse_effective" tells what su_sweep will do.
  *   "fuse_chunk_planes", "fuse_margin", "fuse_cell_planes"   shape of the fused schedule (csrc/fused_schedule.cu).
+ *   "fuse_wait_ns"    wall-clock limit (ns, default 10 s) of one dependency wait inside a fused launch. A correct schedule
+ *                     never comes near it; if a wait does exceed it, that block and every block that waits after it stop
+ *                     WITHOUT storing anything further, and the next synchronising call (su_synchronize, su_plaquette,
+ *                     su_get_counters, ...) returns SU_ECUDA. The links are then a mixture of old and new: the handle
+ *                     drops its fused tables and graphs and counts as uninitialised (SU_ESTATE) until su_init_* /
+ *                     su_import_links / su_load_config. 0 = give up at the first unsuccessful poll (test hook).
  *   "reunit_on_store" 1: su_sweep leaves reunitarised links. Every link is updated exactly once in the last pass of
  *                     a sweep; there the register kernels of Nc <= 4 project the link they have just updated back to
  *                     SU(Nc) before they store it (PAPER.md:143 arithmetic, saving the separate read-modify-write of

@@ -201,7 +201,7 @@ __global__ void k_update_big(const UpdateArgs a, const BigCommon bc) {
         T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
         T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
         const T n2 = r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3;
-        bool ok = have && (n2 > (T)0) && Fn<T>::finite(n2);
+        bool ok = have && (n2 >= Fn<T>::min_norm2()) && Fn<T>::finite(n2);      // as in update_subgroups
         T q4[4] = {(T)1, (T)0, (T)0, (T)0};
         int used = 0;
         const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(0xffffffffu, ok) : 0u;

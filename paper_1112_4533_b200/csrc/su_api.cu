@@ -47,6 +47,7 @@ struct su_lattice {
     int fuse_chunk_planes = 0;       // z-planes per chunk of the fused traversal (0: the plain kernel's Zc)
     int fuse_margin = 8;             // tickets between a cell's last tile and the first tile that depends on it
     int fuse_cell_planes = 0;        // z-planes per cell (0: chosen by fused_make_geom)
+    unsigned long long fuse_wait_ns = 10000000000ull;   // fused launches: a dependency wait longer than this aborts the launch (10 s)
     int prefetch_slices = 0;         // update kernels: L2 prefetch distance in time slices (0: off)
     int blocks_per_sm = 0;           // update kernels: cap on the resident blocks per SM (0: whatever fits)
     int tile_z = 1, tile_t = 1;      // register update kernels: z-planes x time slices per block tile (Geom::Bz, Bt)
@@ -214,6 +215,8 @@ __global__ void k_debug_kp_math(const uint32_t* w, size_t n, double* out) {
     out[5 * i + 4] = Fn<double>::rsqrt_pos(100.0 * u + 1e-3);
 }
 
+void free_graphs(su_lattice* h);
+
 void free_fused(su_lattice* h) {
     for (auto& kv : h->fused) {
         cudaFree(kv.second.d_work); cudaFree(kv.second.d_done); cudaFree(kv.second.d_ctrl);
@@ -286,14 +289,23 @@ su_status fused_table(su_lattice* h, int kind, int sub0, su_lattice::FusedTable*
     return SU_OK;
 }
 
-// a dependency wait that gave up (fused_wait) means a broken schedule: report it instead of returning wrong links
+// A dependency wait that gave up (fused_wait) means a broken schedule or a wedged device: the launch stopped half way,
+// so the links are a mixture of old and new and the tables' counters are inconsistent. Report it, and leave the handle
+// in a state from which the caller can go on: captured graphs and fused tables are dropped (rebuilt and zeroed on the
+// next use) and the lattice counts as uninitialised until su_init_* / su_import_links / su_load_config.
+// Called only after the stream has been synchronised.
 su_status check_fused_error(su_lattice* h) {
+    bool tripped = false;
     for (auto& kv : h->fused) {
         FusedCtrl c{};
         SU_CUDA(h, cudaMemcpy(&c, kv.second.d_ctrl, sizeof(c), cudaMemcpyDeviceToHost), "fused control read-back");
-        if (c.error) return fail(h, SU_ECUDA, "fused launch: a dependency wait timed out; the links are not valid");
+        if (c.error) tripped = true;
     }
-    return SU_OK;
+    if (!tripped) return SU_OK;
+    free_graphs(h);
+    free_fused(h);
+    h->ready = false;
+    return fail(h, SU_ECUDA, "fused launch: a dependency wait timed out; the links are not valid (initialise or import them again)");
 }
 
 // the register kernels of Nc <= 4 can reunitarise the link they have just updated before they store it
@@ -331,6 +343,7 @@ su_status launch_fused_group(su_lattice* h, double beta, int kind, int pass, int
     a.pf_slices = h->prefetch_slices; a.dyn_smem = occupancy_cap_bytes(h);
     a.fz.work = t->d_work; a.fz.done = t->d_done; a.fz.ctrl = t->d_ctrl; a.fz.fg = t->fg; a.fz.fg.sub0 = sub0;
     a.fz.n_tickets = t->n_tickets;
+    a.fz.wait_ns = h->fuse_wait_ns;
     SU_CUDA(h, SU_BY_NC(h, update_nc, h->var, kind, a, h->stream, &h->n_launch), "fused update kernel launch");
     return SU_OK;
 }
@@ -917,17 +930,25 @@ su_status su_load_config(su_lattice* h, const char* path) {
     if (!ok) return fail(h, SU_EINVAL, "su_load_config: '%s' is not a complete configuration file", path);
     if (sum != fnv1a(buf.data(), n * sizeof(double), fnv1a(&hd, sizeof(hd), 14695981039346656037ull)))
         return fail(h, SU_EINVAL, "su_load_config: checksum mismatch in '%s'", path);
+    if ((hd.precision != (int)SU_FP32 && hd.precision != (int)SU_FP64) || (hd.storage != (int)SU_STORE_FULL && hd.storage != (int)SU_STORE_RECON12) ||
+        (hd.storage == (int)SU_STORE_RECON12 && hd.Nc != 3) || hd.reserved != 0 || !std::isfinite(hd.plaquette))
+        return fail(h, SU_EINVAL, "su_load_config: header of '%s' holds values outside their range", path);
+    // Up to here the handle is untouched. The links have to be on the device before their plaquette can be measured,
+    // so a file that fails this last check does overwrite them: the lattice then counts as uninitialised (SU_ESTATE
+    // until su_init_* / su_import_links / another load) instead of silently holding the rejected configuration.
+    // RNG seed and sweep counter are only taken over once everything has passed.
     su_status st = su_import_links(h, buf.data(), n);
-    if (st != SU_OK) return st;
-    st = su_set_rng(h, hd.seed, hd.sweep);
     if (st != SU_OK) return st;
     // the stored plaquette was measured in the writer's precision and storage; a reader in fp32 / two-row storage rounds the links
     double plaq = 0;
     st = su_plaquette(h, &plaq);
-    if (st != SU_OK) return st;
+    if (st != SU_OK) { h->ready = false; return st; }
     const double tol = (h->prec == SU_FP64 && hd.precision == (int)SU_FP64) ? 1e-12 : 1e-5;
-    if (!(std::fabs(plaq - hd.plaquette) <= tol)) return fail(h, SU_EINVAL, "su_load_config: plaquette of '%s' does not match its header", path);
-    return SU_OK;
+    if (!(std::fabs(plaq - hd.plaquette) <= tol)) {
+        h->ready = false;
+        return fail(h, SU_EINVAL, "su_load_config: plaquette of '%s' does not match its header; the lattice is now uninitialised", path);
+    }
+    return su_set_rng(h, hd.seed, hd.sweep);
 }
 
 su_status su_get_counters(su_lattice* h, uint64_t* kp_attempts_total, uint64_t* kp_exhausted) {
@@ -1024,6 +1045,13 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
         (name[0] == 'p' ? h->prefetch_slices : h->blocks_per_sm) = (int)value;
         return SU_OK;
     }
+    if (!strcmp(name, "fuse_wait_ns")) {
+        if (value < 0) return fail(h, SU_EINVAL, "fuse_wait_ns must be >= 0");
+        SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
+        free_graphs(h);                  // the limit is an argument of the captured launches
+        h->fuse_wait_ns = (unsigned long long)value;
+        return SU_OK;
+    }
     const bool is_fuse = !strcmp(name, "fuse"), is_chunk = !strcmp(name, "fuse_chunk_planes"), is_margin = !strcmp(name, "fuse_margin"),
                is_cell = !strcmp(name, "fuse_cell_planes");
     if (is_fuse || is_chunk || is_margin || is_cell) {
@@ -1057,6 +1085,7 @@ su_status su_get_option(su_lattice* h, const char* name, long long* value) {
     if (!strcmp(name, "fuse")) { *value = h->fuse_g; return SU_OK; }
     if (!strcmp(name, "fuse_chunk_planes")) { *value = h->fuse_chunk_planes; return SU_OK; }
     if (!strcmp(name, "fuse_margin")) { *value = h->fuse_margin; return SU_OK; }
+    if (!strcmp(name, "fuse_wait_ns")) { *value = (long long)h->fuse_wait_ns; return SU_OK; }
     if (!strcmp(name, "fuse_cell_planes")) { *value = h->fuse_cell_planes; return SU_OK; }
     if (!strcmp(name, "fuse_effective")) { *value = std::max(effective_fuse(h, 0), effective_fuse(h, 1)); return SU_OK; }
     return fail(h, SU_EINVAL, "su_get_option: unknown option '%s'", name);

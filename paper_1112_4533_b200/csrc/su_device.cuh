@@ -576,6 +576,8 @@ template <> struct Fn<float> {
     static __device__ __forceinline__ float rcp_pos(float x) { return 1.0f / x; }
     static __device__ __forceinline__ float max0(float x) { return fmaxf(x, 0.0f); }
     static __device__ __forceinline__ bool finite(float x) { return isfinite(x); }
+    // smallest k^2 a subgroup update is carried out for (see update_subgroups): below it 1 / k^2 overflows
+    static __device__ __forceinline__ float min_norm2() { return 1.17549435e-38f; }      // FLT_MIN
 };
 template <> struct Fn<double> {
     static __device__ __forceinline__ double log(double x) { return ::log(x); }
@@ -602,6 +604,9 @@ template <> struct Fn<double> {
 #endif
     static __device__ __forceinline__ double max0(double x) { return fmax(x, 0.0); }
     static __device__ __forceinline__ bool finite(double x) { return isfinite(x); }
+    // smallest k^2 a subgroup update is carried out for: rcp / rsqrt.approx.ftz.f64 (the seeds of fast_rcp64 and
+    // fast_rsqrt64) flush a subnormal argument to zero and the Newton steps then turn the infinite seed into NaN
+    static __device__ __forceinline__ double min_norm2() { return 2.2250738585072014e-308; }      // DBL_MIN
 };
 
 // Kennedy-Pendleton draw of v = (a0, a): P(a0) ~ sqrt(1-a0^2) exp(alpha a0) (eq 13),
@@ -745,7 +750,9 @@ __device__ __forceinline__ void update_subgroups(cx<T>* U, cx<T>* W, T beta, uin
             T r0 = (T)0.5 * (wii.re + wjj.re), r1 = (T)0.5 * (wij.im + wji.im);
             T r2 = (T)0.5 * (wij.re - wji.re), r3 = (T)0.5 * (wii.im - wjj.im);
             const T n2 = norm2_4(r0, r1, r2, r3);                        // k^2
-            bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
+            // k = 0 leaves the subgroup unchanged (reading R15); so does a k^2 below the normal range, where 1 / k and
+            // 1 / k^2 are not representable (or not computable by the fast reciprocals): such a block carries no weight
+            bool ok = (n2 >= Fn<T>::min_norm2()) && Fn<T>::finite(n2);
             T a[4] = {(T)1, (T)0, (T)0, (T)0};
             int used = 0;
             const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;

@@ -78,6 +78,7 @@ struct UpdateArgs {
         FusedCtrl* ctrl;               // device
         FusedGeom fg;
         unsigned n_tickets;            // = grid size
+        unsigned long long wait_ns;    // a dependency wait longer than this gives up and aborts the launch (su_set_option "fuse_wait_ns")
     } fz;
 };
 
@@ -449,9 +450,11 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-#ifndef SUG_FUSED_SPIN_LIMIT
-#define SUG_FUSED_SPIN_LIMIT (1u << 20)      // ~0.5 s of polling; a correct schedule never gets near it
-#endif
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 // warp 0 of the block, non-blocking: true iff every dependency of the work item is already complete
 __device__ __forceinline__ bool fused_probe(const UpdateArgs::Fused& fz, int s, int cell, int tile, unsigned epoch) {
     const unsigned target = (epoch + 1u) * (unsigned)fz.fg.nT;
@@ -462,22 +465,30 @@ __device__ __forceinline__ bool fused_probe(const UpdateArgs::Fused& fz, int s, 
     }
     return __all_sync(0xffffffffu, ok);
 }
-// warp 0 of the block: every lane polls some of the work item's dependencies
-__device__ __forceinline__ void fused_wait(const UpdateArgs::Fused& fz, int s, int cell, int tile, unsigned epoch) {
+// warp 0 of the block: every lane polls some of the work item's dependencies. Returns (to every lane) whether they are
+// all complete. false = this wait, or one in another block, lasted longer than fz.wait_ns of WALL-CLOCK time
+// (%globaltimer, so a slow instrumented or debug build does not trip it) and FusedCtrl::error is set: the caller must
+// not run the work item, so that no link computed from incomplete neighbours is ever stored. A correct schedule never
+// gets there; the host reports SU_ECUDA at its next synchronising call and rebuilds the tables (check_fused_error).
+__device__ __forceinline__ bool fused_wait(const UpdateArgs::Fused& fz, int s, int cell, int tile, unsigned epoch) {
     const unsigned target = (epoch + 1u) * (unsigned)fz.fg.nT;
-    for (int k = (int)threadIdx.x; k < s * FUSED_DEPS_PER_STAGE; k += 32) {
+    bool ok = true;
+    unsigned long long t0 = 0;
+    for (int k = (int)threadIdx.x; ok && k < s * FUSED_DEPS_PER_STAGE; k += 32) {
         const int idx = fused_dep(fz.fg, s, cell, tile, k);
         if (idx < 0) continue;
         unsigned spins = 0;
         while ((int)(ld_acquire_u32(fz.done + idx) - target) < 0) {
             __nanosleep(64);
-            ++spins;
-            // give up (and make every other block give up at once) rather than hang the device on a broken schedule
-            if ((spins & 255u) == 0 && *(volatile unsigned*)&fz.ctrl->error) break;
-            if (spins > SUG_FUSED_SPIN_LIMIT) { atomicExch(&fz.ctrl->error, 1u); break; }
+            if ((spins++ & 63u) == 0) {      // on the first unsuccessful poll, then every 64th
+                if (*(volatile unsigned*)&fz.ctrl->error) { ok = false; break; }      // another block gave up: follow at once
+                const unsigned long long now = global_ns();
+                if (t0 == 0) t0 = now;
+                if (now - t0 >= fz.wait_ns) { atomicExch(&fz.ctrl->error, 1u); ok = false; break; }
+            }
         }
     }
-    __syncwarp();
+    return __all_sync(0xffffffffu, ok);
 }
 
 template <int NC, class T, int STORE, int KIND, bool UNR, int BLOCK, int MINB, int FUSE3 = 0, bool KUNR = false, bool FUSED = false>
@@ -503,8 +514,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
                 &s_sm[0][FUSE3 == 4 ? threadIdx.x : 0]);
         }
     } else {
-        __shared__ unsigned sh_ticket, sh_epoch, sh_ready[2];     // sh_ready alternates per phase: no reuse race
+        __shared__ unsigned sh_ticket, sh_epoch, sh_ready[2], sh_abort;     // sh_ready alternates per phase: no reuse race
         if (threadIdx.x == 0) {
+            sh_abort = 0u;
             sh_epoch = *(volatile unsigned*)&a.fz.ctrl->epoch;
             sh_ticket = atomicAdd(&a.fz.ctrl->ticket, 1u);
         }
@@ -522,8 +534,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
         if (st > 0 && st < g) {                                // a block whose first item is not of stage 0 (pipeline drain)
             const uint32_t id = __ldg(work + st);
             const int cell = (int)(id / (unsigned)a.fz.fg.nT);
-            if (threadIdx.x < 32) fused_wait(a.fz, st, cell, (int)(id - (unsigned)cell * (unsigned)a.fz.fg.nT), epoch);
+            if (threadIdx.x < 32) {
+                const bool ok = fused_wait(a.fz, st, cell, (int)(id - (unsigned)cell * (unsigned)a.fz.fg.nT), epoch);
+                if (threadIdx.x == 0 && !ok) sh_abort = 1u;
+            }
             __syncthreads();
+            if (sh_abort) st = g;                              // gave up: run nothing, store nothing
         }
 #pragma unroll 1
         while (st < g) {
@@ -561,8 +577,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) k_update(const UpdateArgs a) {
                 __syncthreads();
                 if (threadIdx.x == BLOCK - 32) { __threadfence(); atomicAdd(a.fz.done + (size_t)st * ncells + cell, 1u); }
                 if (nx < g && !sh_ready[flip]) {               // uniform: written before the barrier
-                    if (threadIdx.x < 32) fused_wait(a.fz, nx, celln, tilen, epoch);
+                    if (threadIdx.x < 32) {
+                        const bool ok = fused_wait(a.fz, nx, celln, tilen, epoch);
+                        if (threadIdx.x == 0 && !ok) sh_abort = 1u;
+                    }
                     __syncthreads();
+                    if (sh_abort) break;                       // gave up: the remaining work items are not run
                 }
             }
             st = nx; flip ^= 1;
@@ -639,7 +659,7 @@ __device__ __forceinline__ void update_link_su2(const UpdateArgs& a, const int p
     qconj(S, A);
     quat_mul(U, A, W);
     const T n2 = norm2_4(W[0], W[1], W[2], W[3]);      // k^2
-    bool ok = (n2 > (T)0) && Fn<T>::finite(n2);
+    bool ok = (n2 >= Fn<T>::min_norm2()) && Fn<T>::finite(n2);      // as in update_subgroups
     int used = 0;
     const unsigned draw_mask = (KIND == KIND_HB) ? __ballot_sync(warp_mask, ok) : 0u;
     if (ok) {

@@ -3,6 +3,7 @@
 // -DSUG_NC=<Nc>. Block size / minimum blocks per SM per variant: DESIGN.md "Launch configuration".
 #include <map>
 #include <mutex>
+#include <tuple>
 
 #include "su_internal.h"
 #include "update_rows_kernel.cuh"
@@ -43,27 +44,39 @@ template <class K> static void launch_k(K kern, unsigned grid, int block, cudaSt
 template <class K> static cudaError_t launch_coop(K kern, unsigned grid, int block, cudaStream_t st, const UpdateArgs& a0) {
     UpdateArgs a = a0;
     if (grid <= 16) {
-        // the whole sub-step is at most 16 blocks: one thread-block cluster, hardware cluster barriers between the sub-steps
+        // the whole sub-step is at most 16 blocks: one thread-block cluster, hardware cluster barriers between the sub-steps.
+        // Whether that cluster can run is decided per (kernel, grid, block) by an occupancy query, not by trying the launch:
+        // the first launch of a handle in graph mode happens inside a stream capture, which a failing launch would
+        // invalidate. The query and the attribute call enqueue nothing, so they are legal during a capture. One mutex
+        // covers the decision, so two host threads never probe the same kernel at once.
         static std::mutex mu;
-        static std::map<const void*, int> state;          // 0 unknown, 1 cluster launches work for this kernel, -1 they do not
+        static std::map<std::tuple<const void*, unsigned, int>, int> state;      // 1: cluster launches work for this configuration, -1: not
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = grid; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
         int st_k;
-        { std::lock_guard<std::mutex> lock(mu); st_k = state[(const void*)kern]; }
-        if (st_k == 0) {
-            st_k = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess ? 1 : -1;
-            cudaGetLastError();
+        {
+            std::lock_guard<std::mutex> lock(mu);
+            int& known = state[std::make_tuple((const void*)kern, grid, block)];
+            if (known == 0) {
+                int n_clusters = 0;
+                const bool ok = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess &&
+                                cudaOccupancyMaxActiveClusters(&n_clusters, kern, &cfg) == cudaSuccess && n_clusters >= 1;
+                cudaGetLastError();
+                known = ok ? 1 : -1;
+            }
+            st_k = known;
         }
         if (st_k == 1) {
-            cudaLaunchConfig_t cfg{};
-            cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-            cudaLaunchAttribute attr[1];
-            attr[0].id = cudaLaunchAttributeClusterDimension;
-            attr[0].val.clusterDim.x = grid; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-            cfg.attrs = attr; cfg.numAttrs = 1;
             a.coop_cluster = 1;
             const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, a);
-            { std::lock_guard<std::mutex> lock(mu); state[(const void*)kern] = e == cudaSuccess ? 1 : -1; }
             if (e == cudaSuccess) return e;
-            cudaGetLastError();                           // e.g. the cluster does not fit: fall back to the grid barrier
+            cudaGetLastError();                           // against the query's answer: this configuration only falls back to the grid barrier
+            std::lock_guard<std::mutex> lock(mu);
+            state[std::make_tuple((const void*)kern, grid, block)] = -1;
         }
     }
     a.coop_cluster = 0;

@@ -150,3 +150,48 @@ def test_fused_sweep_at_full_size_is_bitwise_the_plain_sweep(mods, precision, g)
     out = B.export_links()
     for i in range(0, 48, 8):
         assert np.array_equal(out[i:i + 8], ref[i:i + 8])
+
+
+def test_a_dependency_wait_that_gives_up_stores_nothing_more_and_the_handle_recovers(mods):
+    """su_set_option "fuse_wait_ns" = 0: a wait that does not find its dependencies complete at its first poll gives
+    up, exactly what a wait beyond the 10 s default does. The launch must then be reported (SU_ECUDA at the next
+    synchronising call), the handle must refuse to go on with the half-updated links (SU_ESTATE), and after a new
+    import with the default limit the fused sweep must again be bitwise the plain one (tables rebuilt and zeroed)."""
+    su, _ = mods
+    dims = (16, 16, 16, 16)
+    A = su.Lattice(3, dims, "fp64")
+    A.init_hot(21)
+    start = A.export_links()
+    A.sweep(6.0, 1, 2)
+    want = A.export_links()
+
+    B = su.Lattice(3, dims, "fp64")
+    B.set_option("fuse", 8)
+    B.set_option("fuse_margin", 1)                   # dependent tiles as close together as the schedule allows: blocks do wait
+    default_ns = B.get_option("fuse_wait_ns")
+    assert default_ns == 10_000_000_000
+    B.set_option("fuse_wait_ns", 0)
+    tripped = False
+    for _ in range(8):                               # in practice the first sweep already has a block that has to wait
+        B.import_links(start)
+        B.set_rng(21, 0)
+        B.sweep(6.0, 1, 2)
+        try:
+            B.synchronize()
+        except su.SuError as e:
+            assert e.status == su.SU_ECUDA and "dependency wait timed out" in str(e)
+            tripped = True
+            break
+    assert tripped, "no fused block ever had to wait: the give-up path was not exercised"
+    with pytest.raises(su.SuError) as e:
+        B.sweep(6.0, 1, 2)
+    assert e.value.status == su.SU_ESTATE
+    with pytest.raises(su.SuError) as e:
+        B.plaquette()
+    assert e.value.status == su.SU_ESTATE
+    B.set_option("fuse_wait_ns", default_ns)
+    B.import_links(start)
+    B.set_rng(21, 0)
+    B.sweep(6.0, 1, 2)
+    B.synchronize()
+    assert np.array_equal(B.export_links(), want)

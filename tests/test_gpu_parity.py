@@ -478,6 +478,34 @@ def test_configuration_file_roundtrip_and_exact_resume(mods, tmp_path):
         su.Lattice(3, DIMS_ANISO).save_config(tmp_path / "x.sug")
     assert e.value.status == su.SU_ESTATE
 
+    # files whose checksum is right but whose header is not (a writer bug, or a file edited and re-signed)
+    def resigned(edit):
+        import struct
+        body = bytearray(path.read_bytes()[:-8])
+        edit(body, struct)
+        hsh = 14695981039346656037
+        for b in bytes(body):
+            hsh = ((hsh ^ b) * 1099511628211) & 0xFFFFFFFFFFFFFFFF
+        out = tmp_path / "resigned.sug"
+        out.write_bytes(bytes(body) + struct.pack("<Q", hsh))
+        return out
+
+    before, seed_sweep_probe = B.export_links(), B.plaquette()
+    with pytest.raises(su.SuError) as e:                              # precision field out of range: refused, handle untouched
+        B.load_config(resigned(lambda b, st: b.__setitem__(slice(28, 32), st.pack("<i", 7))))
+    assert e.value.status == su.SU_EINVAL and "range" in str(e.value)
+    assert np.array_equal(B.export_links(), before) and B.plaquette() == seed_sweep_probe
+    with pytest.raises(su.SuError) as e:                              # wrong plaquette: links already overwritten -> uninitialised
+        B.load_config(resigned(lambda b, st: b.__setitem__(slice(56, 64), st.pack("<d", 0.123))))
+    assert e.value.status == su.SU_EINVAL and "does not match its header" in str(e.value)
+    for call in (B.plaquette, lambda: B.sweep(6.0, 1, 2), B.export_links):
+        with pytest.raises(su.SuError) as e:
+            call()
+        assert e.value.status == su.SU_ESTATE
+    B.load_config(path)                                               # a good file makes the handle usable again
+    B.sweep(6.0, 1, 2)
+    assert np.array_equal(A.export_links(), B.export_links())
+
 
 @pytest.mark.parametrize("v", [(2, "fp64", False, "auto"), (3, "fp64", False, "auto"), (3, "fp64", True, "auto"), (3, "fp32", False, "auto"),
                                (4, "fp64", False, "auto"), (6, "fp64", False, "auto"), (3, "fp64", False, "generic")], ids=_ids)
@@ -601,6 +629,32 @@ def test_cooperative_whole_pass_launches_are_bitwise_the_plain_sweep(mods, v, di
             assert got[3] <= 3 * 3, got[3]                       # two launches per sweep (+ the graph's counter node) instead of 40
 
 
+def test_first_sweep_of_a_process_may_be_a_graph_capture_of_the_cluster_launch(mods):
+    """The decision "can this sub-step run as one thread-block cluster" is taken by an occupancy query, so it is safe
+    when the very first update launch of a process happens inside a CUDA-graph capture (no other test has that order:
+    the decision is cached per process). A fresh interpreter: graph mode + coop_sweep from the first sweep on, 8^4
+    (16 blocks per sub-step = one cluster), against a plain lattice in the same process, bitwise."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import numpy as np, paper_1112_4533_b200 as su\n"
+        "G = su.Lattice(2, (8, 8, 8, 8), 'fp64', graph=True)\n"
+        "G.set_option('coop_sweep', 1)\n"
+        "G.init_hot(3)\n"
+        "for _ in range(3): G.sweep(2.3, 1, 2)\n"          # the first call captures, the next two replay
+        "G.synchronize()\n"
+        "assert G.get_option('coop_sweep_effective') == 3\n"
+        "P = su.Lattice(2, (8, 8, 8, 8), 'fp64')\n"
+        "P.init_hot(3)\n"
+        "for _ in range(3): P.sweep(2.3, 1, 2)\n"
+        "assert np.array_equal(G.export_links(), P.export_links())\n"
+        "print('ok')\n")
+    r = subprocess.run([sys.executable, "-c", code], cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and r.stdout.strip().endswith("ok"), r.stdout + r.stderr
+
+
 def test_cooperative_launch_falls_back_when_the_lattice_does_not_fit(mods):
     su, _ = mods
     G = su.Lattice(3, (32, 32, 32, 32), "fp64")                  # 524288 sites per parity: far more than one wave of blocks
@@ -636,3 +690,32 @@ def test_fast_math_against_host(mods):
     assert (np.abs(got[:, 3] - np.sqrt(u)) / np.sqrt(u)).max() < 3e-16
     x = 100 * u + np.longdouble(1e-3)
     assert (np.abs(got[:, 4] * np.sqrt(x) - 1)).max() < 4e-16
+
+
+@pytest.mark.parametrize("Nc,precision,kernel", [(2, "fp64", "auto"), (3, "fp64", "auto"), (3, "fp32", "auto"), (4, "fp64", "auto"),
+                                                 (3, "fp64", "generic"), (6, "fp64", "auto"), (9, "fp64", "auto")],
+                         ids=lambda v: str(v))
+def test_subnormal_subgroup_norm_leaves_the_link_unchanged(mods, Nc, precision, kernel):
+    """Reading R15, extended: a subgroup block of W = U S^dagger whose k^2 lies below the normal range of the
+    arithmetic is treated like k = 0 (that subgroup is skipped; heatbath counts it in kp_exhausted). 1 / k^2 is not
+    representable there in fp32, and the fp64 kernels' reciprocal seeds (rcp / rsqrt.approx.ftz.f64) flush such an
+    argument to zero: without the guard every link of the sub-step came out NaN. Links scaled so that k^2 ~ s^8 is
+    subnormal (products of up to four links stay normal)."""
+    su, _ = mods
+    dims = (4, 4, 4, 6)
+    s = 3.2e-40 if precision == "fp64" else 7.5e-6
+    rng = np.random.default_rng(77 + Nc)
+    links = H.random_links(rng, Nc, dims) * s
+    G = su.Lattice(Nc, dims, precision, False, kernel)
+    G.import_links(links)
+    before = G.export_links()
+    assert np.all(np.isfinite(before.view(np.float64))) and np.abs(before).max() > 0
+    for kind in (1, 0):                                  # overrelaxation, then heatbath
+        for parity in range(2):
+            for mu in range(4):
+                G.substep(BETA.get(Nc, 60.0), kind, 0, parity, mu)
+        after = G.export_links()
+        assert np.all(np.isfinite(after.view(np.float64)))
+        assert np.array_equal(after, before)
+    attempts, exhausted = G.counters()
+    assert attempts == 0 and exhausted == 4 * int(np.prod(dims)) * (Nc * (Nc - 1) // 2)
