@@ -373,6 +373,75 @@ def test_hot_start_is_haar_like(Nc):
     assert np.abs(L2.export_links() - links).max() > 0.1
 
 
+def _hot_link_restated(Nc, dims, seed, site, mu):
+    """One hot-start link written out from the documented keying (SURVEY.md 8(c) "Hot start"; DESIGN.md "RNG keying";
+    PAPER.md:164), sharing nothing with the oracle: Philox counter (c0, c1, c2, c3) = (lexicographic site, 0,
+    kind 2 << 28 | parity << 19 | mu << 17, block b), key = (seed low, seed high) through the big-integer Philox of
+    tests/test_oracle_rng.py (itself pinned by the published known-answer vectors); the four words of block b are two
+    Box-Muller pairs (u_a, u_b) -> sqrt(-2 ln u_a) (cos, sin)(2 pi u_b) with u = (w + 1) / 2^32; the Gaussians fill the
+    Nc x Nc complex matrix row-major as (re, im); Gram-Schmidt over ROWS with positive normalisation = the QR
+    factorisation of the transpose with a positive diagonal (LAPACK, not the oracle's loop); last row times
+    conj(det) / |det|. SU(2): the first four Gaussians, normalised, are (a0..a3) of eq 6."""
+    from test_oracle_rng import _philox_bigint
+    Lx, Ly, Lz, Lt = dims
+    x = site % Lx; y = (site // Lx) % Ly; z = (site // (Lx * Ly)) % Lz; t = site // (Lx * Ly * Lz)
+    parity = (x + y + z + t) & 1
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    ng = 4 if Nc == 2 else 2 * Nc * Nc
+    g = []
+    for b in range((ng + 3) // 4):
+        w = _philox_bigint((site, 0, (2 << 28) | (parity << 19) | (mu << 17), b), key)
+        for ua, ub in ((w[0], w[1]), (w[2], w[3])):
+            rad = np.sqrt(-2.0 * np.log((ua + 1) / 2.0 ** 32))
+            ang = 2.0 * np.pi * ((ub + 1) / 2.0 ** 32)
+            g += [rad * np.cos(ang), rad * np.sin(ang)]
+    g = np.array(g)
+    if Nc == 2:
+        a = g[:4] / np.linalg.norm(g[:4])
+        return np.array([[a[0] + 1j * a[3], a[2] + 1j * a[1]], [-a[2] + 1j * a[1], a[0] - 1j * a[3]]])
+    M = (g[0:ng:2] + 1j * g[1:ng:2]).reshape(Nc, Nc)
+    Q, R = np.linalg.qr(M.T)
+    d = np.diagonal(R)
+    U = (Q * (d / np.abs(d))).T                       # rows of U: the orthonormalised rows of M, positive normalisation
+    det = np.linalg.det(U)
+    U[Nc - 1] *= np.conj(det) / abs(det)
+    return U
+
+
+@pytest.mark.parametrize("Nc", [2, 3, 4])
+@pytest.mark.parametrize("seed", [1, (1 << 40) + 12345])
+def test_hot_start_keying_against_an_independent_restatement(Nc, seed):
+    """Pins WHICH random numbers make WHICH link (a hot start that reused one matrix for the four
+    directions of a site, or one site's matrix for its neighbour, passed every Haar-moment test)."""
+    dims = (4, 6, 2, 4)
+    L = oracle.OracleLattice(Nc, dims)
+    L.init_hot(seed)
+    links = L.export_links()                          # [t][z][y][x][mu][row][col]
+    flat = links.reshape(-1, 4, Nc, Nc)               # lexicographic site, x fastest
+    V = flat.shape[0]
+    rng = np.random.default_rng(5)
+    sites = sorted(set([0, 1, dims[0], V - 1] + [int(s) for s in rng.integers(0, V, 8)]))
+    for site in sites:
+        for mu in range(4):
+            want = _hot_link_restated(Nc, dims, seed, site, mu)
+            assert np.abs(flat[site, mu] - want).max() < 1e-13, (site, mu)
+    # independent draws: the four links of a site, and the same direction on neighbouring sites, are different matrices
+    for site in sites:
+        for mu in range(4):
+            for nu in range(mu + 1, 4):
+                assert np.abs(flat[site, mu] - flat[site, nu]).max() > 1e-2
+            assert np.abs(flat[site, mu] - flat[(site + 1) % V, mu]).max() > 1e-2
+    # the seed's high word is part of the key
+    if seed >> 32:
+        L2 = oracle.OracleLattice(Nc, dims)
+        L2.init_hot(seed & 0xFFFFFFFF)
+        assert np.abs(L2.export_links() - links).max() > 0.1
+    # fp32 lattices hold the same matrices rounded to float (reading R20)
+    L32 = oracle.OracleLattice(Nc, dims, "fp32")
+    L32.init_hot(seed)
+    assert np.abs(L32.export_links() - links).max() < 1e-7
+
+
 @pytest.mark.parametrize("Nc", [2, 3, 4, 5])
 def test_reunitarize(Nc):
     dims = (2, 2, 2, 4)
