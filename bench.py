@@ -146,6 +146,40 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def sustained_copy(torch, device_index, seconds=0.6, nbytes=1 << 30):
+    """What a pure-DRAM kernel keeps on THIS box for as long as a timed step runs: device-to-device copies of 1 GiB
+    (cudaMemcpyAsync through torch's copy_, read + write = 2 GiB of traffic each), back to back for `seconds`, CUDA events
+    around all of them, clocks and power sampled meanwhile. MEASURED_PEAKS.json's figure is the best of ten single
+    copies (a burst); the update kernels are timed inside a 0.3 - 0.6 s run at the board's power cap, so this is the
+    denominator of the same regime (measurement item 7)."""
+    dev = torch.device("cuda", device_index)
+    a = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    b = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    a.zero_()
+    for _ in range(3):
+        b.copy_(a)
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); b.copy_(a); e1.record(); torch.cuda.synchronize(dev)
+    one_ms = max(e0.elapsed_time(e1), 1e-3)
+    n = max(10, int(seconds * 1e3 / one_ms))
+    sampler = ClockSampler(device_index)
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(n):
+        b.copy_(a)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    t1 = time.perf_counter()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(t0, t1)
+    del a, b
+    torch.cuda.empty_cache()
+    return {"gbs": 2.0 * nbytes * n / (ms * 1e-3) / 1e9, "single_copy_gbs": 2.0 * nbytes / (one_ms * 1e-3) / 1e9, "copies": n,
+            "bytes_per_copy": nbytes, "seconds": ms * 1e-3, "clocks": clocks,
+            "how": "torch copy_ (cudaMemcpyAsync D2D) of 1 GiB, back to back, CUDA events, read + write bytes"}
+
+
 def rank_seed(wl, rank):
     """N > 1 runs independent replicas: rank r's Markov chain is seeded seed + r."""
     return wl["seed"] + rank
@@ -751,6 +785,13 @@ def main():
                              "hb_launch_ms": n["roofline"]["hb_avg_launch_ms"] if n["roofline"] else None})
             l2.close()
             del l2
+
+    if rank == 0 and main_num["roofline"] is not None:
+        sc = sustained_copy(torch, local)
+        roof = main_num["roofline"]
+        roof["hbm"]["sustained_copy_gbs"] = sc["gbs"]
+        roof["hbm"]["frac_of_sustained_copy"] = roof["hbm"]["achieved_gbs"] / sc["gbs"]
+        roof["sustained_copy"] = sc
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -199,6 +199,9 @@ su_status su_slab_plaquette_sum(su_lattice* const* slabs, int n_slabs, double* o
  *                     su_reunitarize); the other kernels run the reunitarisation kernel at the end of the sweep. This
  *                     one DOES change results at rounding level against su_sweep + su_reunitarize (later sub-steps of
  *                     the last pass already see projected neighbours); su_sweep without it never reunitarises. 0: off.
+ *   "substep_reunit"  test hook, 1: su_substep runs the kernel instances of that last pass (the link is projected back to
+ *                     SU(Nc) right before it is stored), so that they can be compared with the reference sub-step by
+ *                     sub-step. Register kernels of Nc <= 4 only (else SU_EUNSUPPORTED). Does not affect su_sweep.
  *   "coop_sweep"      1: su_sweep runs all heatbath passes of a sweep in ONE cooperative launch and all overrelaxation
  *                     passes in another, with grid barriers where the launch boundaries were (register kernels of
  *                     Nc <= 4, lattices whose V/2 threads are resident at once, not slabs; otherwise plain launches;

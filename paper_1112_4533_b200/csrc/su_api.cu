@@ -53,6 +53,7 @@ struct su_lattice {
     int tile_z = 1, tile_t = 1;      // register update kernels: z-planes x time slices per block tile (Geom::Bz, Bt)
     bool coop_sweep = false;         // su_sweep: one cooperative launch per kind (all its passes) when the lattice fits the device at once
     long long coop_sites[2] = {-1, -1};   // cached capacity (sites of one parity) of the cooperative kernel per kind; -1: not queried
+    bool substep_reunit = false;     // test hook: su_substep runs the reunitarise-before-store kernel instances (the last pass of a reunit_on_store sweep)
     bool reunit_on_store = false;    // su_sweep leaves reunitarised links (in its last pass; see su_set_option)                     // slab mode: false between su_import_links and su_slab_halo_push
     uint64_t seed = 0;
     uint32_t sweep = 0;
@@ -767,7 +768,7 @@ su_status su_substep(su_lattice* h, double beta, int kind, int pass, int parity,
         }
         SU_CUDA(h, cudaMemsetAsync(h->d_attempts, 0, nbytes, h->stream), "attempt buffer reset");
     }
-    su_status st = launch_substep(h, beta, kind, pass, parity, mu, host_attempts ? h->d_attempts : nullptr, nullptr);
+    su_status st = launch_substep(h, beta, kind, pass, parity, mu, host_attempts ? h->d_attempts : nullptr, nullptr, h->substep_reunit);
     if (st != SU_OK) return st;
     if (host_attempts) {
         SU_CUDA(h, cudaMemcpyAsync(host_attempts, h->d_attempts, nbytes, cudaMemcpyDeviceToHost, h->stream), "attempt copy");
@@ -1045,6 +1046,12 @@ su_status su_set_option(su_lattice* h, const char* name, long long value) {
         (name[0] == 'p' ? h->prefetch_slices : h->blocks_per_sm) = (int)value;
         return SU_OK;
     }
+    if (!strcmp(name, "substep_reunit")) {
+        if (value != 0 && value != 1) return fail(h, SU_EINVAL, "substep_reunit must be 0 or 1");
+        if (value && !reunit_in_kernel(h)) return fail(h, SU_EUNSUPPORTED, "substep_reunit: only the register kernels of Nc <= 4 reunitarise before the store");
+        h->substep_reunit = value != 0;
+        return SU_OK;
+    }
     if (!strcmp(name, "fuse_wait_ns")) {
         if (value < 0) return fail(h, SU_EINVAL, "fuse_wait_ns must be >= 0");
         SU_CUDA(h, cudaStreamSynchronize(h->stream), "su_set_option");
@@ -1086,6 +1093,7 @@ su_status su_get_option(su_lattice* h, const char* name, long long* value) {
     if (!strcmp(name, "fuse_chunk_planes")) { *value = h->fuse_chunk_planes; return SU_OK; }
     if (!strcmp(name, "fuse_margin")) { *value = h->fuse_margin; return SU_OK; }
     if (!strcmp(name, "fuse_wait_ns")) { *value = (long long)h->fuse_wait_ns; return SU_OK; }
+    if (!strcmp(name, "substep_reunit")) { *value = h->substep_reunit ? 1 : 0; return SU_OK; }
     if (!strcmp(name, "fuse_cell_planes")) { *value = h->fuse_cell_planes; return SU_OK; }
     if (!strcmp(name, "fuse_effective")) { *value = std::max(effective_fuse(h, 0), effective_fuse(h, 1)); return SU_OK; }
     return fail(h, SU_EINVAL, "su_get_option: unknown option '%s'", name);

@@ -50,8 +50,8 @@ def _maxdiff(a, b, chunk=1 << 20):
     return m
 
 
-@pytest.mark.parametrize("precision,recon12", [("fp64", False), ("fp32", False), ("fp64", True)],
-                         ids=["fp64-full", "fp32-full", "fp64-r12"])
+@pytest.mark.parametrize("precision,recon12", [("fp64", False), ("fp32", False), ("fp64", True), ("fp32", True)],
+                         ids=["fp64-full", "fp32-full", "fp64-r12", "fp32-r12"])      # the four variants bench.py times
 def test_su3_48_substeps_every_link(mods, precision, recon12):
     su, oracle = mods
     dims = (L_FULL,) * 4

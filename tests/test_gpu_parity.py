@@ -119,6 +119,61 @@ def test_lockstep_substeps_over_one_sweep(mods, v):
     assert abs(ga - oa) <= 2 * flipped
 
 
+REUNIT_VARIANTS = [(3, "fp64", False), (3, "fp32", False), (3, "fp64", True), (3, "fp32", True), (4, "fp64", False),
+                   (4, "fp32", False), (2, "fp64", False), (2, "fp32", False)]
+
+
+@pytest.mark.parametrize("v", REUNIT_VARIANTS, ids=lambda v: f"su{v[0]}-{v[1]}-{'r12' if v[2] else 'full'}")
+def test_lockstep_substeps_of_the_reunitarise_on_store_kernels(mods, v):
+    """The gate of the kernel instances that bench.py times (su_set_option "reunit_on_store": in the last pass of a sweep
+    the register kernels project the link they have just updated back to SU(Nc) before they store it). Driven sub-step
+    by sub-step through su_substep with the test hook "substep_reunit", against the oracle's sub-step followed by the
+    oracle's reunitarisation OF THE LINKS JUST UPDATED (all others keep their bits: export, reunitarise, export, merge,
+    import - oracle arithmetic only). Every link, fp64 <= 1e-11, fp32 <= 2e-5 with the Kennedy-Pendleton decision flips
+    counted, re-synchronised after each sub-step like the plain lock-step test; one heatbath and one overrelaxation pass."""
+    Nc, precision, recon12 = v
+    G, O = _pair(mods, Nc, DIMS_ANISO, precision, recon12, "auto")
+    _thermalised_oracle(O, Nc)
+    lo = O.export_links()
+    G.import_links(lo)
+    G.set_option("substep_reunit", 1)
+    assert G.get_option("substep_reunit") == 1
+    G.set_rng(11, 3)
+    O.set_rng(11, 3)
+    beta = BETA[Nc]
+    updated = flipped = 0
+    for kind, pass_, parity, mu in _schedule(1, 1):
+        ag = G.substep(beta, kind, pass_, parity, mu, want_attempts=True)
+        ao = O.substep(beta, kind, pass_, parity, mu, want_attempts=True)
+        raw = O.export_links()
+        O.reunitarize()
+        merged = raw.copy()
+        site_of_cb = _sites_of_parity(DIMS_ANISO, parity)
+        merged.reshape(-1, 4, Nc, Nc)[site_of_cb, mu] = O.export_links().reshape(-1, 4, Nc, Nc)[site_of_cb, mu]
+        O.import_links(merged)
+        lo = O.export_links()
+        assert np.array_equal(lo, merged) or recon12        # two-row storage rebuilds the third row on import
+        lg = G.export_links()
+        d = np.abs(lg - lo).reshape(-1, 4, Nc * Nc).max(axis=2)
+        flip_site = np.zeros(O.V, dtype=bool)
+        if kind == 0:
+            flip_site[site_of_cb[(ag != ao).any(axis=0)]] = True
+        updated += O.V // 2
+        flipped += int(flip_site.sum())
+        assert d[~flip_site].max() <= TOL[precision], (kind, parity, mu, float(d[~flip_site].max()))
+        if precision == "fp64":
+            assert not flip_site.any()
+        # the links that were just stored are in the group; they differ from the unprojected update at rounding level only
+        upd = lg.reshape(-1, 4, Nc, Nc)[site_of_cb, mu]
+        tol_group = 1e-13 if precision == "fp64" else 1e-6
+        assert H.unitarity_defect(upd) < tol_group and H.det_defect(upd) < tol_group
+        G.import_links(lo)
+    assert flipped <= max(1, int(1e-5 * updated)), (flipped, updated)
+    with pytest.raises(mods[0].SuError) as e:
+        mods[0].Lattice(6, (4, 4, 4, 4), "fp64").set_option("substep_reunit", 1)
+    assert e.value.status == mods[0].SU_EUNSUPPORTED
+
+
 def _sites_of_parity(dims, parity):
     Lx, Ly, Lz, Lt = dims
     t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
@@ -532,6 +587,8 @@ def test_reunitarise_on_store(mods, v):
     O.sweep(BETA[Nc], 1, 2)
     O.reunitarize()
     G.reunitarize()
+    # fp32: a whole sweep without re-synchronisation is not a gate (a flipped Kennedy-Pendleton decision changes a link
+    # at O(1)); the fp32 gate of these kernel instances is test_lockstep_substeps_of_the_reunitarise_on_store_kernels
     tol = 1e-11 if precision == "fp64" else 1e-3
     assert np.abs(G.export_links() - O.export_links()).max() <= tol
     # a damaged link is repaired by the sweep itself
