@@ -657,7 +657,7 @@ def variant_numbers(wl, precision, recon12, res, steps, n_ranks, peak):
                 "hb_alu_frac": (flops_per_update(Nc, "hb", recon12) * (V // 2) / (hb_ms * 1e-3) / 1e12 / alu_peak) if hb_ms and alu_peak else None,
                 "update_kernels_share_of_step": ((or_ms * N_OR * 8 + (hb_ms or 0.0) * N_HB * 8) / (res["ms"] / steps)),
                 "traffic": ncu_traffic(f"su{Nc}_{precision}_{'recon12' if recon12 else 'full'}_or"),
-                "traffic_source": "profiles/traffic.csv (ncu --set full of this kernel, committed; not re-measured in this run)"}
+                "traffic_source": "profiles/traffic.csv (round-3 ncu capture of this kernel, profiles/r03a_traffic_and_sustained_copy.md; not re-measured in this run)"}
         # Third figure: the L2 -> SM read path. A link update issues 19 link loads (18 staple links + the own link) and L1
         # serves < 10 % of them, so ~19 R s bytes per update cross the L2 fabric, 2.1 x the 9 R s that must cross HBM. The
         # path delivers 11 kB per SM clock chip-wide (su_measure_l2_peak, = 94 % of the 11.8 kB / clock ncu states), and the
