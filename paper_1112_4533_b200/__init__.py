@@ -24,7 +24,7 @@ SU_STORE_FULL, SU_STORE_RECON12 = 0, 1
 SU_KERNEL_AUTO, SU_KERNEL_SPECIALISED, SU_KERNEL_GENERIC = 0, 1, 2
 SU_MAX_NC = 32
 
-# every entry point include/su_gauge.h declares (tests check the library exports exactly these)
+# every entry point include/su_gauge.h and include/su_gauge_test.h declare (tests check the library exports exactly these)
 ABI_SYMBOLS = (
     "su_lattice_bytes", "su_lattice_create", "su_lattice_create_ex", "su_lattice_destroy",
     "su_init_cold", "su_init_hot", "su_sweep", "su_plaquette", "su_polyakov", "su_reunitarize",

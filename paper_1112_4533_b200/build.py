@@ -22,7 +22,8 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
 ]
-HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", "update_rows_kernel.cuh", "fused_schedule.h", os.path.join("..", "..", "include", "su_gauge.h")]
+HEADERS = ["su_device.cuh", "su_internal.h", "update_kernel.cuh", "update_rows_kernel.cuh", "fused_schedule.h", os.path.join("..", "..", "include", "su_gauge.h"),
+           os.path.join("..", "..", "include", "su_gauge_test.h")]
 
 
 def _units():

@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "../../include/su_gauge.h"
+#include "../../include/su_gauge_test.h"
 #include "su_device.cuh"
 #include "update_kernel.cuh"
 

@@ -9,12 +9,24 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "su_gauge.h")
+TEST_HEADER = os.path.join(ROOT, "include", "su_gauge_test.h")      # micro-benchmarks and test hooks: not product interface
+TEST_ONLY = ["su_debug_kp_math", "su_fused_dep_debug", "su_fused_schedule_debug", "su_measure_fma_peak", "su_measure_l2_peak"]
+
+
+def _names(path):
+    text = open(path).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(su_[a-z0-9_]+)\s*\(", text)))
 
 
 def _declared():
-    text = open(HEADER).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(su_[a-z0-9_]+)\s*\(", text)))
+    return sorted(_names(HEADER) + _names(TEST_HEADER))
+
+
+def test_product_header_holds_no_benchmark_or_debug_entry_point():
+    assert _names(TEST_HEADER) == TEST_ONLY
+    assert not set(_names(HEADER)) & set(TEST_ONLY)
+    assert not [n for n in _names(HEADER) if "debug" in n or "measure" in n]
 
 
 @pytest.fixture(scope="module")
